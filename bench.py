@@ -1,0 +1,306 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the He-4 VMC hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--mode fp32c|fp64]
+                    [--sweeps-per-step m] [--impl ours|reference] [--no-cpu-baseline]
+
+One STEP = the whole hot path over all walkers of the workload: m Metropolis sweeps (default 1)
++ one local-energy evaluation + the acceptance read-out.
+Default workload: BASELINE.json configs[2] = N = 1952 atoms, 2048 walkers, fp32 coordinates with
+fp64 sums, the configuration the metric is quoted on.  Prints ONE JSON line (see DESIGN.md
+"Measurement" for every key).  --impl reference times the CPU oracle on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1312_1282_b200 import workloads as wl  # noqa: E402
+
+# Algorithmic FP instructions per u-evaluation of the sweep: thread-level
+# instructions on the pipe that bounds the mode, for ONE trial-position pair evaluation.
+ALG_INSTR = {wl.MODE_FP32C: 24.0, wl.MODE_FP64: 31.0}
+LANES_PER_SM = {wl.MODE_FP32C: 128, wl.MODE_FP64: 64}
+
+
+def pair_counts(w: wl.Workload, m: int):
+    """(sweep pair evaluations, energy pairs) per step over all walkers: N(N-1) per walker-sweep
+    (one trial evaluation per (moved, other) pair) and N(N-1)/2 per energy evaluation."""
+    N, W = w.n_atoms, w.n_walkers
+    return W * m * N * (N - 1), W * N * (N - 1) // 2
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons during the timed region (nvidia-smi, 5 Hz)."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+
+    def run(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        while not self._stop_evt.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                f = [x.strip() for x in out.strip().split(",")]
+                self.samples.append(float(f[0]))
+                self.max_mhz = float(f[1])
+                for n, v in zip(names, f[2:6]):
+                    if v.lower().startswith("active"):
+                        self.reasons.add(n)
+            except Exception:
+                pass
+            self._stop_evt.wait(0.2)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=10)
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def cpu_baseline(w: wl.Workload, m: int, budget_s: float = 12.0):
+    """The oracle as it stands on the host cores: one OS thread per walker, `cores` walkers of the
+    same workload (same seed, so a subset of the GPU run's chains), whole steps until ~budget_s."""
+    import oracle
+    cores = oracle.num_threads()
+    N, g = w.n_atoms, w.groups[0]
+    s = oracle.System(N, w.box_L[0], g.b, w.hbar2_over_2m, w.aziz)
+    x = oracle.init_walkers(s, w.seed, 0, cores, wl.JITTER)
+    oracle.sweep(s, x[:1].copy(), w.seed, 0, 0, 0, g.step)          # load/compile outside the timing
+    steps, t0, t = 0, time.perf_counter(), 0
+    while True:
+        oracle.sweep(s, x, w.seed, 0, t, m, g.step)
+        oracle.local_energy(s, x)
+        t += m
+        steps += 1
+        el = time.perf_counter() - t0
+        if el >= budget_s or steps >= 50:
+            break
+    pairs = steps * cores * (m * N * (N - 1) + N * (N - 1) // 2)
+    return {"value": pairs / el, "unit": "pair-evals/s", "cores": cores, "kind": "oracle",
+            "sample": f"{cores} walkers x {steps} steps (m={m} sweeps + 1 energy) of {w.name}, fp64, {el:.1f} s wall",
+            "walker_sweeps_per_s": steps * cores * m / el, "ms_per_step_sample": 1e3 * el / steps}
+
+
+def run_reference(args, w, m):
+    """--impl reference: the reference arm for this tier is the CPU oracle (no reference code exists)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    cores = oracle.num_threads()
+    N, g = w.n_atoms, w.groups[0]
+    s = oracle.System(N, w.box_L[0], g.b, w.hbar2_over_2m, w.aziz)
+    x = oracle.init_walkers(s, w.seed, 0, cores, wl.JITTER)
+    t = 0
+    for _ in range(args.warmup):
+        oracle.sweep(s, x, w.seed, 0, t, m, g.step)
+        oracle.local_energy(s, x)
+        t += m
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.sweep(s, x, w.seed, 0, t, m, g.step)
+        oracle.local_energy(s, x)
+        t += m
+    el = time.perf_counter() - t0
+    pairs = args.steps * cores * (m * N * (N - 1) + N * (N - 1) // 2)
+    val = pairs / el
+    sample = f"each step = {cores} walkers (one per core) of {w.name}: m={m} sweeps + 1 energy, fp64 oracle"
+    print(json.dumps({
+        "impl": "reference", "metric": "pair evaluations/s (sweep N(N-1) + energy N(N-1)/2 per walker-step)",
+        "value": val, "unit": "pair-evals/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "N": N, "walkers_per_step": cores, "sweeps_per_step": m, "mode": "oracle-fp64"},
+        "cpu_baseline": {"value": val, "unit": "pair-evals/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "pair-evals/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "walker_sweeps_per_s": args.steps * cores * m / el,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--mode", choices=["fp32c", "fp64", "default"], default="default")
+    ap.add_argument("--sweeps-per-step", type=int, default=1)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--walkers", type=int, default=None, help="truncate walkers per group (debugging)")
+    args = ap.parse_args()
+
+    w = wl.config(args.config)
+    if args.mode != "default":
+        w = wl.with_mode(w, wl.MODE_FP64 if args.mode == "fp64" else wl.MODE_FP32C)
+    if args.walkers:
+        w = w.truncated(args.walkers)
+    m = args.sweeps_per_step
+    if args.impl == "reference":
+        if args.steps is None:
+            args.steps = 5
+        return run_reference(args, w, m)
+    if args.steps is None:
+        args.steps = 20
+
+    import torch
+    import torch.distributed as dist
+    from paper_1312_1282_b200 import binding
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+
+    # weak scaling: every rank runs the workload's W walkers; global walker ids continue across ranks
+    W, N = w.n_walkers, w.n_atoms
+    q = binding.QMC(N, w.walkers_per_group, w.box_L, w.jastrow_b, w.hbar2_over_2m, w.aziz, w.mode,
+                    walker_id_base=rank * W, jitter=wl.JITTER, device=str(dev))
+    q.init_walkers(w.seed)
+    steps = w.steps
+    e_out = torch.empty((W, 4), dtype=torch.float64, device=dev)
+    a_out = torch.empty((W,), dtype=torch.float64, device=dev)
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)   # 256 MiB > 126 MB L2
+
+    def one_step():
+        q.sweep(m, steps)
+        q.local_energy(e_out)
+        q.acceptance(a_out)
+
+    for _ in range(args.warmup):
+        one_step()
+    torch.cuda.synchronize()
+
+    K = args.steps
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+    sampler = ClockSampler(local) if rank == 0 else None
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    launches0 = q.info()["kernel_launches"]
+    for k in range(K):
+        flush.zero_()                                   # L2 flush between timed iterations (untimed)
+        ev[k][0].record()
+        q.sweep(m, steps)
+        ev[k][1].record()
+        q.local_energy(e_out)
+        q.acceptance(a_out)
+        ev[k][2].record()
+    torch.cuda.synchronize()
+    launches = q.info()["kernel_launches"] - launches0
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop() if sampler else None
+    t_sweep = sum(ev[k][0].elapsed_time(ev[k][1]) for k in range(K)) * 1e-3
+    t_total = sum(ev[k][0].elapsed_time(ev[k][2]) for k in range(K)) * 1e-3
+    if world > 1:
+        tt = torch.tensor([t_total, t_sweep], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_total, t_sweep = float(tt[0]), float(tt[1])
+    acc = float(a_out.mean())
+    e_mean = (e_out.mean(0) / N).tolist()
+
+    # ---- end to end through the host-buffer call (rank-local, same walkers) -------------------
+    h_in = q.get_positions().cpu().pin_memory()
+    h_e = torch.empty((W, 4), dtype=torch.float64).pin_memory()
+    h_a = torch.empty((W,), dtype=torch.float64).pin_memory()
+    h_x = torch.empty((W, 3, N), dtype=torch.float64).pin_memory()
+    Ke = max(3, min(K, 10))
+    q.step_host(m, steps, h_in, h_e, h_a, h_x)          # warm-up
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        q.step_host(m, steps, h_x, h_e, h_a, h_x)       # coordinates in, energies + coordinates out
+    t_e2e = time.perf_counter() - t0
+    if world > 1:
+        tt = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_e2e = float(tt[0])
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    sweep_pairs, energy_pairs = pair_counts(w, m)
+    pairs_step = sweep_pairs + energy_pairs
+    value = world * K * pairs_step / t_total
+    info = q.info()
+    mode_name = "fp32c" if w.mode == wl.MODE_FP32C else "fp64"
+
+    # ---- roofline of the dominant kernel (the sweep): plain-ALU bound ---------------------------
+    peak_meas = binding.pipe_peak(0 if w.mode == wl.MODE_FP64 else 1)
+    sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
+    peak_derived = info["sm_count"] * LANES_PER_SM[w.mode] * sm_max * 1e6        # lane-instr/s
+    t_launch = t_sweep / K
+    achieved = sweep_pairs * ALG_INSTR[w.mode] / t_launch
+    executed = sweep_pairs * (1.0 + acc) * ALG_INSTR[w.mode] / t_launch
+    roofline = {
+        "bound": "alu", "kernel": f"sweep_kernel<{mode_name}>",
+        "achieved": achieved / 1e9, "peak": peak_derived / 1e9, "unit": "G thread-instr/s",
+        "frac": achieved / peak_derived, "traffic": None,
+        "peak_source": f"derived: {info['sm_count']} SMs x {LANES_PER_SM[w.mode]} lanes x {sm_max:.0f} MHz (DESIGN.md)",
+        "peak_measured_fma_chain": peak_meas / 1e9,
+        "alg_instr_per_pair_eval": ALG_INSTR[w.mode],
+        "executed_frac": executed / peak_derived,
+        "note": "achieved counts ONE trial evaluation per (moved, other) pair; executed_frac adds the "
+                "accepted-move re-evaluations the running-sum update performs (x(1+acceptance))",
+        "kernel_ms": 1e3 * t_launch,
+    }
+
+    out = {
+        "metric": "pair evaluations/s (sweep N(N-1) + energy N(N-1)/2 per walker-step)",
+        "value": value, "unit": "pair-evals/s", "n_gpus": world, "steps": K, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if w.mode == wl.MODE_FP32C else "f64", "data": "synthetic",
+        "config": {"workload": w.name, "N": N, "walkers_per_gpu": W, "groups": len(w.groups),
+                   "sweeps_per_step": m, "mode": mode_name, "energy_every_step": True,
+                   "l2": "flushed between timed steps (256 MiB write, untimed)",
+                   "sweep_threads": info["sweep_threads"], "sweep_ctas_per_sm": info["sweep_ctas_per_sm"],
+                   "energy_threads": info["energy_threads"], "energy_ctas_per_sm": info["energy_ctas_per_sm"]},
+        "walker_sweeps_per_s": world * K * W * m / t_total,
+        "sweep_only": {"pair_evals_per_s": world * K * sweep_pairs / t_sweep,
+                       "walker_sweeps_per_s": world * K * W * m / t_sweep, "ms": 1e3 * t_sweep / K,
+                       "u_evals_executed_per_s": world * K * sweep_pairs * (1 + acc) / t_sweep},
+        "energy_only": {"pairs_per_s": world * K * energy_pairs / (t_total - t_sweep),
+                        "ms": 1e3 * (t_total - t_sweep) / K},
+        "acceptance": acc, "energy_per_atom_K": dict(zip(["E_PB", "V", "T_PB", "T_JF"], e_mean)),
+        "clocks": clocks,
+        "e2e": {"value": world * Ke * pairs_step / t_e2e, "unit": "pair-evals/s",
+                "h2d_bytes_per_step": W * 3 * N * 8, "d2h_bytes_per_step": W * 3 * N * 8 + W * 5 * 8,
+                "ms_per_step": 1e3 * t_e2e / Ke, "api": "qmc_step_host (pinned host buffers)"},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+    }
+    if not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(w, m)
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

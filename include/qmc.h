@@ -1,0 +1,139 @@
+/*
+ * qmc.h -- C ABI of the B200-native He-4 variational Monte Carlo hot path.
+ *
+ * Implements the per-walker Metropolis sweep of single-particle moves and the
+ * local-energy estimator of "Fast quantum Monte Carlo on a GPU" (arXiv:1312.1282;
+ * citations below are PAPER.md line numbers, "Rn" are the readings in DESIGN.md).
+ *
+ * Conventions
+ *  - Plain C, no C++ or torch types.  Every call returns QMC_OK (0) or a negative
+ *    qmc_status; nothing aborts or throws.  qmc_last_error() gives a message.
+ *  - "device" pointers are CUDA device memory owned by the CALLER (e.g. a torch
+ *    tensor's data_ptr()); "host" pointers are ordinary host memory (pinned memory
+ *    makes the *_host calls asynchronous copies).  The library never frees them.
+ *  - All work is enqueued on the CUDA stream given to qmc_create (a cudaStream_t
+ *    passed as void*; NULL = legacy default stream) and is asynchronous with respect
+ *    to the host, except qmc_create / qmc_destroy and the *_host calls (which
+ *    synchronise the stream before returning).
+ *  - Units: Angstrom and Kelvin.  Coordinates are SoA per walker: xyz[w][c][i],
+ *    c = 0,1,2, i = 0..N-1, i.e. [W][3][N] doubles, wrapped into [0, L].
+ *  - Walkers are independent Markov chains (l.169); walker w of this context has
+ *    global id walker_id_base + w, which keys its random stream, so a shard of a
+ *    larger run reproduces exactly the walkers it owns.
+ */
+#ifndef QMC_B200_H
+#define QMC_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qmc_ctx qmc_ctx;   /* opaque; owned by the library */
+
+typedef enum {
+    QMC_OK = 0,
+    QMC_E_ARG = -1,        /* bad argument (NULL, N < 2, step >= L/2, ...)                 */
+    QMC_E_CAPACITY = -2,   /* N does not fit the mode's per-CTA shared-memory budget        */
+    QMC_E_CUDA = -3,       /* a CUDA runtime call failed (message in qmc_last_error)        */
+    QMC_E_STATE = -4       /* call order (e.g. sweep before init_walkers/set_positions)     */
+} qmc_status;
+
+typedef enum {
+    QMC_FP64 = 0,          /* fp64 coordinates and arithmetic throughout                    */
+    QMC_FP32C = 1          /* fp32 coordinates + pair arithmetic, fp64 sums (R20)           */
+} qmc_mode;
+
+/* Problem statement (l.319 inputs; l.410 run-time fields bulkdimarray, jastrowb, mass).
+ * Host memory; copied by qmc_create, the caller keeps ownership. */
+typedef struct {
+    int32_t        N;                 /* atoms per walker, >= 2                                   */
+    int32_t        n_groups;          /* parameter points in this context (>= 1)                  */
+    const int32_t *walkers_per_group; /* [n_groups]; W = sum; walkers are numbered group by group */
+    const double  *box_L;             /* [n_groups] cubic box edge L (l.460); cutoff is L/2       */
+    const double  *jastrow_b;         /* [n_groups] b of Eq.(9) l.155                             */
+    double         hbar2_over_2m;     /* K*A^2                                                    */
+    double         aziz[9];           /* HFD-B(HE) l.131: eps, rm, A, alpha, beta, c6, c8, c10, D  */
+    int32_t        mode;              /* qmc_mode                                                 */
+    uint32_t       walker_id_base;    /* global id of this context's walker 0                     */
+    double         jitter;            /* half-width of the initial lattice jitter (R13)           */
+} qmc_params;
+
+/* Bytes of device memory the walker state of `p` needs (coordinates, per-particle pair
+ * sums S_i, counters).  0 on invalid parameters. */
+size_t qmc_state_bytes(const qmc_params *p);
+
+/* Create a context.  d_state: caller-owned device buffer of >= qmc_state_bytes(p) bytes,
+ * 256-byte aligned, which must outlive the context; or NULL to let the library allocate
+ * (cudaMalloc) and free it.  Validates parameters, precomputes per-group constants.
+ * Errors: QMC_E_ARG, QMC_E_CAPACITY (e.g. N = 10000 in QMC_FP64), QMC_E_CUDA. */
+int qmc_create(const qmc_params *p, void *cuda_stream, void *d_state, size_t state_bytes, qmc_ctx **out);
+int qmc_destroy(qmc_ctx *c);
+
+/* Jittered FCC start (R13), pair sums S_i built, counters and sweep index t set to 0. */
+int qmc_init_walkers(qmc_ctx *c, uint64_t seed);
+
+/* n_sweeps Metropolis sweeps of every walker (Eq.(5) l.123, Eq.(7) l.146, l.325-331): for each
+ * sweep t, for s = 0..N-1: trial r_s + delta with delta uniform in [-step,step]^3 from
+ * Philox4x32-10(counter (s,t,walker id,0), key seed); accept iff 2*Delta > log(xi); on accept
+ * commit the wrapped position and update the running pair sums.  steps: HOST array [n_groups]
+ * (one step per parameter point), 0 < step < L/2.  Successive calls continue t:
+ * sweep(a); sweep(b) == sweep(a+b). */
+int qmc_sweep(qmc_ctx *c, int32_t n_sweeps, const double *steps);
+
+/* Local energy of every walker's current configuration (l.113-115, l.129, l.381):
+ * d_out: device [W][4] = E_PB, V, T_PB, T_JF, totals in K (divide by N for per-atom).
+ * Also rebuilds the running pair sums S_i from scratch (R17). */
+int qmc_local_energy(qmc_ctx *c, double *d_out);
+
+/* d_out: device [W] accepted / attempted moves since qmc_init_walkers / qmc_set_positions. */
+int qmc_acceptance(qmc_ctx *c, double *d_out);
+
+/* One whole step with HOST buffers (the paper's block cycle, l.319-343: coordinates in,
+ * sweeps, energies and coordinates written out).  Any pointer may be NULL to skip that part.
+ * h_xyz_in [W][3][N] is uploaded first (and S_i rebuilt); then n_sweeps sweeps; then the local
+ * energy -> h_energy [W][4], acceptance -> h_acc [W], coordinates -> h_xyz_out [W][3][N].
+ * Synchronises the stream before returning. */
+int qmc_step_host(qmc_ctx *c, const double *h_xyz_in, int32_t n_sweeps, const double *steps,
+                  double *h_energy, double *h_acc, double *h_xyz_out);
+
+/* Message for the last error of this context (or of the last failed qmc_create if c is NULL).
+ * Library-owned, valid until the next call. */
+const char *qmc_last_error(const qmc_ctx *c);
+
+/* ---- state access and parity hooks (not on the timed path) -------------------------------- */
+int qmc_get_positions(qmc_ctx *c, double *d_xyz);        /* device [W][3][N], exact widening in FP32C */
+int qmc_set_positions(qmc_ctx *c, const double *d_xyz);  /* device [W][3][N]; rebuilds S_i, zeroes counters,
+                                                            keeps the sweep index t and the seed          */
+int qmc_set_seed(qmc_ctx *c, uint64_t seed, uint32_t t); /* random key and sweep index for the next sweep  */
+int qmc_get_pair_sums(qmc_ctx *c, double *d_S);          /* device [W][N] running S_i                      */
+int qmc_refresh_pair_sums(qmc_ctx *c);                   /* S_i <- sum_{j != i} u(r_ij) from scratch       */
+/* Record, for walkers w_begin <= w < w_end, one byte per move (1 = accepted) and the decision
+ * margin 2*Delta - log(xi) of the following qmc_sweep calls, starting at move 0 of the buffers:
+ * d_dec device [(w_end-w_begin)][moves_capacity] uint8, d_margin same shape double (may be NULL).
+ * Pass d_dec = NULL to stop recording. */
+int qmc_trace_decisions(qmc_ctx *c, int32_t w_begin, int32_t w_end, uint8_t *d_dec, double *d_margin,
+                        int64_t moves_capacity);
+
+/* ---- introspection ------------------------------------------------------------------------ */
+typedef struct {
+    int32_t W, N, n_groups, mode;
+    int32_t sweep_threads, sweep_ctas_per_sm, sweep_smem_bytes, sweep_pairs_per_thread;
+    int32_t energy_threads, energy_ctas_per_sm, energy_smem_bytes;
+    int32_t sm_count;
+    uint32_t t;                       /* sweeps done since init                        */
+    uint64_t kernel_launches;         /* kernels this context has launched so far      */
+} qmc_info_t;
+int qmc_info(const qmc_ctx *c, qmc_info_t *out);
+
+/* FP pipe peak microbenchmark: runs a dependent-chain-free FMA kernel on
+ * every SM and reports thread-level FMA instructions per second (host out, synchronous).
+ * which: 0 = fp64 DFMA, 1 = fp32 FFMA. */
+int qmc_pipe_peak(int32_t which, void *cuda_stream, double *h_fma_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QMC_B200_H */

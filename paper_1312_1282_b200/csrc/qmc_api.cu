@@ -1,0 +1,521 @@
+// qmc_api.cu -- the C ABI of include/qmc.h: context management, small state kernels
+// (initial lattice, position import/export, acceptance), host-buffer step, pipe-peak microbenchmark.
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "qmc_internal.h"
+
+using namespace qmc;
+
+static char g_create_err[512] = "no error";
+
+#define QMC_FAIL(c, code, ...)                                         \
+    do {                                                               \
+        snprintf((c) ? (c)->err : g_create_err, 512, __VA_ARGS__);     \
+        return (code);                                                 \
+    } while (0)
+
+#define QMC_CUDA(c, expr)                                                                     \
+    do {                                                                                      \
+        cudaError_t e__ = (expr);                                                             \
+        if (e__ != cudaSuccess) QMC_FAIL(c, QMC_E_CUDA, "%s: %s", #expr, cudaGetErrorString(e__)); \
+    } while (0)
+
+namespace qmc {
+
+// ------------------------------------------------------------------------------------------
+// Initial walkers (R13): particle i on FCC site floor(i*M/N), M = 4k^3, sites ordered
+// (ix,iy,iz,basis) with the basis fastest; + jitter * a_c, a_c from Philox counter (i,0,walker,1).
+// ------------------------------------------------------------------------------------------
+template <typename Real>
+__global__ void init_kernel(StateView sv, uint2 key, double jitter)
+{
+    const int N = sv.N, ld = sv.ld;
+    const int w = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const GroupDev g = sv.groups[sv.group_of[w]];
+    const long long k = g.k_lat, M = 4 * k * k * k;
+    const long long site = ((long long)i * M) / N;
+    const int bas = (int)(site & 3);
+    const long long cell = site >> 2;
+    const long long iz = cell % k, iy = (cell / k) % k, ix = cell / (k * k);
+    const double ox = (bas == 1 || bas == 2) ? 0.5 : 0.0;
+    const double oy = (bas == 1 || bas == 3) ? 0.5 : 0.0;
+    const double oz = (bas == 2 || bas == 3) ? 0.5 : 0.0;
+    const uint4 r = philox4x32_10(make_uint4((uint32_t)i, 0u, sv.walker_id_base + (uint32_t)w, 1u), key);
+    const double idx[3] = {(double)ix + ox, (double)iy + oy, (double)iz + oz};
+    const uint32_t word[3] = {r.x, r.y, r.z};
+    Real *pos = reinterpret_cast<Real *>(sv.pos) + (size_t)w * 3 * ld;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double v = __dadd_rn(__dmul_rn(idx[c], g.a_lat), __dmul_rn(jitter, word_to_pm1(word[c])));
+        if (v >= g.L) v = __dadd_rn(v, -g.L);
+        if (v < 0.0) v = __dadd_rn(v, g.L);
+        Real q = (Real)v;
+        const Real Lr = (Real)g.L;                 // FP32C: keep the stored value inside [0, L_fp32]
+        if (q >= Lr) q -= Lr;
+        if (q < (Real)0) q += Lr;
+        pos[c * ld + i] = q;
+    }
+}
+
+template <typename Real>
+__global__ void set_positions_kernel(StateView sv, const double *__restrict__ xyz)
+{
+    const int N = sv.N, ld = sv.ld;
+    const int w = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ld) return;
+    Real *pos = reinterpret_cast<Real *>(sv.pos) + (size_t)w * 3 * ld;
+    const double *src = xyz + (size_t)w * 3 * N;
+    const Real Lr = (Real)sv.groups[sv.group_of[w]].L;
+    for (int c = 0; c < 3; ++c) {
+        Real q = (Real)0;
+        if (i < N) {
+            q = (Real)src[c * N + i];
+            if (q >= Lr) q -= Lr;
+            if (q < (Real)0) q += Lr;
+        }
+        pos[c * ld + i] = q;
+    }
+    if (i == 0) sv.n_acc[w] = 0ull;
+}
+
+template <typename Real>
+__global__ void get_positions_kernel(StateView sv, double *__restrict__ xyz)
+{
+    const int N = sv.N, ld = sv.ld;
+    const int w = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const Real *pos = reinterpret_cast<const Real *>(sv.pos) + (size_t)w * 3 * ld;
+    double *dst = xyz + (size_t)w * 3 * N;
+    for (int c = 0; c < 3; ++c) dst[c * N + i] = (double)pos[c * ld + i];
+}
+
+__global__ void get_pair_sums_kernel(StateView sv, double *__restrict__ S)
+{
+    const int w = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < sv.N) S[(size_t)w * sv.N + i] = sv.S[(size_t)w * sv.ld + i];
+}
+
+__global__ void acceptance_kernel(StateView sv, double attempted, double *__restrict__ out)
+{
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w < sv.W) out[w] = attempted > 0.0 ? (double)sv.n_acc[w] / attempted : 0.0;
+}
+
+__global__ void zero_state_kernel(StateView sv, size_t pos_bytes)
+{
+    // zero the padding of every row once so that vector copies never move uninitialised bytes
+    const size_t n = pos_bytes / 4;
+    uint32_t *p = reinterpret_cast<uint32_t *>(sv.pos);
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = 0u;
+    double *S = sv.S;
+    const size_t ns = (size_t)sv.W * sv.ld;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < ns; i += (size_t)gridDim.x * blockDim.x) S[i] = 0.0;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < (size_t)sv.W; i += (size_t)gridDim.x * blockDim.x) sv.n_acc[i] = 0ull;
+}
+
+static dim3 grid_wn(const qmc_ctx *c, int n) { return dim3((unsigned)((n + 127) / 128), (unsigned)c->W); }
+
+cudaError_t launch_init(qmc_ctx *c)
+{
+    c->launches += 1;
+    const uint2 key = make_uint2((uint32_t)(c->seed & 0xFFFFFFFFull), (uint32_t)(c->seed >> 32));
+    if (c->p.mode == QMC_FP64) init_kernel<double><<<grid_wn(c, c->p.N), 128, 0, c->stream>>>(c->sv, key, c->p.jitter);
+    else                       init_kernel<float><<<grid_wn(c, c->p.N), 128, 0, c->stream>>>(c->sv, key, c->p.jitter);
+    return cudaGetLastError();
+}
+cudaError_t launch_set_positions(qmc_ctx *c, const double *d_xyz)
+{
+    c->launches += 1;
+    if (c->p.mode == QMC_FP64) set_positions_kernel<double><<<grid_wn(c, c->ld), 128, 0, c->stream>>>(c->sv, d_xyz);
+    else                       set_positions_kernel<float><<<grid_wn(c, c->ld), 128, 0, c->stream>>>(c->sv, d_xyz);
+    return cudaGetLastError();
+}
+cudaError_t launch_get_positions(qmc_ctx *c, double *d_xyz)
+{
+    c->launches += 1;
+    if (c->p.mode == QMC_FP64) get_positions_kernel<double><<<grid_wn(c, c->p.N), 128, 0, c->stream>>>(c->sv, d_xyz);
+    else                       get_positions_kernel<float><<<grid_wn(c, c->p.N), 128, 0, c->stream>>>(c->sv, d_xyz);
+    return cudaGetLastError();
+}
+cudaError_t launch_acceptance(qmc_ctx *c, double *d_out)
+{
+    c->launches += 1;
+    acceptance_kernel<<<(c->W + 127) / 128, 128, 0, c->stream>>>(c->sv, (double)(c->t - c->t_acc0) * (double)c->p.N, d_out);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// FP pipe peak: 8 independent FMA chains per thread, 2048 threads per SM, no memory traffic.
+// ------------------------------------------------------------------------------------------
+template <typename Real>
+__global__ void __launch_bounds__(256) fma_peak_kernel(Real *sink, int iters, Real a, Real b)
+{
+    Real v[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k] = (Real)(threadIdx.x + k);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int rep = 0; rep < 8; ++rep)
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = fma(v[k], a, b);
+    }
+    Real s = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += v[k];
+    if (s == (Real)123456789) sink[0] = s;      // never true; keeps the chains alive
+}
+
+}  // namespace qmc
+
+// ==========================================================================================
+// C ABI
+// ==========================================================================================
+static bool valid_params(const qmc_params *p, char *err)
+{
+    if (!p) { snprintf(err, 512, "params is NULL"); return false; }
+    if (p->N < 2) { snprintf(err, 512, "N must be >= 2 (got %d)", p->N); return false; }
+    if (p->n_groups < 1 || !p->walkers_per_group || !p->box_L || !p->jastrow_b) {
+        snprintf(err, 512, "n_groups >= 1 and the three per-group arrays are required"); return false;
+    }
+    if (p->mode != QMC_FP64 && p->mode != QMC_FP32C) { snprintf(err, 512, "unknown mode %d", p->mode); return false; }
+    long long W = 0;
+    for (int g = 0; g < p->n_groups; ++g) {
+        if (p->walkers_per_group[g] < 0) { snprintf(err, 512, "walkers_per_group[%d] < 0", g); return false; }
+        if (!(p->box_L[g] > 0.0) || !(p->jastrow_b[g] >= 0.0)) { snprintf(err, 512, "box_L > 0 and jastrow_b >= 0 required (group %d)", g); return false; }
+        W += p->walkers_per_group[g];
+    }
+    if (W < 1 || W > 0x7fffffffLL) { snprintf(err, 512, "total walker count %lld out of range", W); return false; }
+    if (!(p->aziz[1] > 0.0)) { snprintf(err, 512, "aziz r_m must be > 0"); return false; }
+    return true;
+}
+
+static int round_up4(int n) { return (n + 3) & ~3; }
+
+static void state_layout(const qmc_params *p, long long W, size_t *pos_bytes, size_t *S_off, size_t *acc_off, size_t *total)
+{
+    const size_t ld = (size_t)round_up4(p->N);
+    const size_t real = p->mode == QMC_FP64 ? 8 : 4;
+    auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
+    *pos_bytes = (size_t)W * 3 * ld * real;
+    *S_off = up(*pos_bytes);
+    *acc_off = up(*S_off + (size_t)W * ld * 8);
+    *total = up(*acc_off + (size_t)W * 8);
+}
+
+extern "C" size_t qmc_state_bytes(const qmc_params *p)
+{
+    char err[512];
+    if (!valid_params(p, err)) return 0;
+    long long W = 0;
+    for (int g = 0; g < p->n_groups; ++g) W += p->walkers_per_group[g];
+    size_t pb, so, ao, tot;
+    state_layout(p, W, &pb, &so, &ao, &tot);
+    return tot;
+}
+
+extern "C" int qmc_create(const qmc_params *p, void *cuda_stream, void *d_state, size_t state_bytes, qmc_ctx **out)
+{
+    if (!out) QMC_FAIL((qmc_ctx *)nullptr, QMC_E_ARG, "out is NULL");
+    *out = nullptr;
+    if (!valid_params(p, g_create_err)) return QMC_E_ARG;
+    qmc_ctx *c = new (std::nothrow) qmc_ctx();
+    if (!c) QMC_FAIL((qmc_ctx *)nullptr, QMC_E_ARG, "out of host memory");
+    c->p = *p;
+    c->walkers_per_group.assign(p->walkers_per_group, p->walkers_per_group + p->n_groups);
+    c->box_L.assign(p->box_L, p->box_L + p->n_groups);
+    c->jastrow_b.assign(p->jastrow_b, p->jastrow_b + p->n_groups);
+    c->p.walkers_per_group = c->walkers_per_group.data();
+    c->p.box_L = c->box_L.data();
+    c->p.jastrow_b = c->jastrow_b.data();
+    c->stream = (cudaStream_t)cuda_stream;
+    c->ld = round_up4(p->N);
+    long long W = 0;
+    for (int g = 0; g < p->n_groups; ++g) W += p->walkers_per_group[g];
+    c->W = (int32_t)W;
+
+#define CREATE_FAIL(code, ...) do { snprintf(g_create_err, 512, __VA_ARGS__); qmc_destroy(c); return (code); } while (0)
+#define CREATE_CUDA(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) CREATE_FAIL(QMC_E_CUDA, "%s: %s", #expr, cudaGetErrorString(e__)); } while (0)
+
+    int dev = 0;
+    CREATE_CUDA(cudaGetDevice(&dev));
+    CREATE_CUDA(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev));
+
+    // per-group constants
+    c->groups.resize(p->n_groups);
+    for (int g = 0; g < p->n_groups; ++g) {
+        GroupDev &G = c->groups[g];
+        const double L = p->box_L[g], b = p->jastrow_b[g];
+        G.L = L; G.h = 0.5 * L; G.h2 = G.h * G.h;
+        G.b5 = b * b * b * b * b;
+        G.c1 = -0.5 * G.b5;
+        const double h = G.h;
+        G.c0 = G.b5 / (h * h * h * h * h);
+        G.step = 0.0;
+        long long k = 1;
+        while (4 * k * k * k < p->N) ++k;
+        G.k_lat = (int32_t)k;
+        G.a_lat = L / (double)k;
+        G.pad = 0;
+    }
+    const double *a = p->aziz;
+    c->aziz.eps = a[0]; c->aziz.inv_rm = 1.0 / a[1]; c->aziz.rm2 = a[1] * a[1]; c->aziz.A = a[2];
+    c->aziz.alpha = a[3]; c->aziz.beta = a[4]; c->aziz.c6 = a[5]; c->aziz.c8 = a[6]; c->aziz.c10 = a[7];
+    c->aziz.D = a[8]; c->aziz.Drm = a[8] * a[1];
+
+    // state buffer
+    size_t pos_bytes, S_off, acc_off, total;
+    state_layout(p, W, &pos_bytes, &S_off, &acc_off, &total);
+    if (d_state) {
+        if (state_bytes < total) CREATE_FAIL(QMC_E_ARG, "state buffer too small: %zu < %zu bytes", state_bytes, total);
+        if (((uintptr_t)d_state & 255) != 0) CREATE_FAIL(QMC_E_ARG, "state buffer must be 256-byte aligned");
+        c->d_state = d_state;
+    } else {
+        CREATE_CUDA(cudaMalloc(&c->d_state, total));
+        c->owns_state = true;
+    }
+    std::vector<int32_t> group_of((size_t)W);
+    {
+        size_t w = 0;
+        for (int g = 0; g < p->n_groups; ++g)
+            for (int k = 0; k < p->walkers_per_group[g]; ++k) group_of[w++] = g;
+    }
+    CREATE_CUDA(cudaMalloc(&c->d_groups, sizeof(GroupDev) * p->n_groups));
+    CREATE_CUDA(cudaMalloc(&c->d_group_of, sizeof(int32_t) * (size_t)W));
+    CREATE_CUDA(cudaMalloc(&c->d_scratch, sizeof(double) * ((size_t)W * 5 + (size_t)W * 3 * p->N)));
+    CREATE_CUDA(cudaMemcpyAsync(c->d_groups, c->groups.data(), sizeof(GroupDev) * p->n_groups, cudaMemcpyHostToDevice, c->stream));
+    CREATE_CUDA(cudaMemcpyAsync(c->d_group_of, group_of.data(), sizeof(int32_t) * (size_t)W, cudaMemcpyHostToDevice, c->stream));
+    CREATE_CUDA(cudaStreamSynchronize(c->stream));
+
+    c->sv.pos = c->d_state;
+    c->sv.S = reinterpret_cast<double *>((char *)c->d_state + S_off);
+    c->sv.n_acc = reinterpret_cast<unsigned long long *>((char *)c->d_state + acc_off);
+    c->sv.group_of = c->d_group_of;
+    c->sv.groups = c->d_groups;
+    c->sv.W = c->W; c->sv.N = p->N; c->sv.ld = c->ld;
+    c->sv.walker_id_base = p->walker_id_base;
+
+    if (!plan_sweep(c, &c->sweep_plan))
+        CREATE_FAIL(QMC_E_CAPACITY, "N = %d does not fit the sweep kernel's shared-memory budget in mode %d "
+                    "(needs %d bytes per CTA, limit %d)", p->N, p->mode, c->sweep_plan.smem_bytes, 227 * 1024);
+    if (!plan_energy(c, &c->energy_plan))
+        CREATE_FAIL(QMC_E_CAPACITY, "N = %d does not fit the energy kernel's shared-memory budget in mode %d", p->N, p->mode);
+
+    zero_state_kernel<<<c->sm_count * 4, 256, 0, c->stream>>>(c->sv, pos_bytes);
+    CREATE_CUDA(cudaGetLastError());
+    CREATE_CUDA(cudaStreamSynchronize(c->stream));
+    c->launches += 1;
+    *out = c;
+    snprintf(g_create_err, 512, "no error");
+    return QMC_OK;
+}
+
+extern "C" int qmc_destroy(qmc_ctx *c)
+{
+    if (!c) return QMC_OK;
+    cudaStreamSynchronize(c->stream);
+    if (c->owns_state && c->d_state) cudaFree(c->d_state);
+    if (c->d_groups) cudaFree(c->d_groups);
+    if (c->d_group_of) cudaFree(c->d_group_of);
+    if (c->d_scratch) cudaFree(c->d_scratch);
+    delete c;
+    return QMC_OK;
+}
+
+extern "C" const char *qmc_last_error(const qmc_ctx *c) { return c ? c->err : g_create_err; }
+
+extern "C" int qmc_init_walkers(qmc_ctx *c, uint64_t seed)
+{
+    if (!c) return QMC_E_ARG;
+    c->seed = seed;
+    c->t = 0;
+    c->t_acc0 = 0;
+    c->trace.offset = 0;
+    QMC_CUDA(c, cudaMemsetAsync(c->sv.n_acc, 0, sizeof(unsigned long long) * (size_t)c->W, c->stream));
+    QMC_CUDA(c, launch_init(c));
+    QMC_CUDA(c, launch_energy(c, nullptr, false));       // build S_i
+    c->have_state = true;
+    return QMC_OK;
+}
+
+extern "C" int qmc_set_seed(qmc_ctx *c, uint64_t seed, uint32_t t)
+{
+    if (!c) return QMC_E_ARG;
+    c->seed = seed;
+    c->t_acc0 += t - c->t;       // keep the attempted-move count of qmc_acceptance unchanged
+    c->t = t;
+    return QMC_OK;
+}
+
+extern "C" int qmc_sweep(qmc_ctx *c, int32_t n_sweeps, const double *steps)
+{
+    if (!c) return QMC_E_ARG;
+    if (!c->have_state) QMC_FAIL(c, QMC_E_STATE, "qmc_sweep before qmc_init_walkers / qmc_set_positions");
+    if (n_sweeps < 0 || !steps) QMC_FAIL(c, QMC_E_ARG, "n_sweeps >= 0 and steps != NULL required");
+    if (n_sweeps == 0) return QMC_OK;
+    bool changed = false;
+    for (int g = 0; g < c->p.n_groups; ++g) {
+        if (!(steps[g] > 0.0) || !(steps[g] < 0.5 * c->box_L[g]))
+            QMC_FAIL(c, QMC_E_ARG, "steps[%d] = %g must lie in (0, L/2 = %g)", g, steps[g], 0.5 * c->box_L[g]);
+        if (c->groups[g].step != steps[g]) { c->groups[g].step = steps[g]; changed = true; }
+    }
+    if (changed)   // stream-ordered update of the small constant table (host mirror is ours, pageable copy is synchronous to the host)
+        QMC_CUDA(c, cudaMemcpyAsync(c->d_groups, c->groups.data(), sizeof(GroupDev) * c->p.n_groups, cudaMemcpyHostToDevice, c->stream));
+    QMC_CUDA(c, launch_sweep(c, n_sweeps));
+    c->t += (uint32_t)n_sweeps;
+    if (c->trace.dec) c->trace.offset += (long long)n_sweeps * c->p.N;
+    return QMC_OK;
+}
+
+extern "C" int qmc_local_energy(qmc_ctx *c, double *d_out)
+{
+    if (!c || !d_out) return QMC_E_ARG;
+    if (!c->have_state) QMC_FAIL(c, QMC_E_STATE, "qmc_local_energy before qmc_init_walkers / qmc_set_positions");
+    QMC_CUDA(c, launch_energy(c, d_out, true));
+    return QMC_OK;
+}
+
+extern "C" int qmc_refresh_pair_sums(qmc_ctx *c)
+{
+    if (!c) return QMC_E_ARG;
+    if (!c->have_state) QMC_FAIL(c, QMC_E_STATE, "no walker state yet");
+    QMC_CUDA(c, launch_energy(c, nullptr, false));
+    return QMC_OK;
+}
+
+extern "C" int qmc_acceptance(qmc_ctx *c, double *d_out)
+{
+    if (!c || !d_out) return QMC_E_ARG;
+    QMC_CUDA(c, launch_acceptance(c, d_out));
+    return QMC_OK;
+}
+
+extern "C" int qmc_get_positions(qmc_ctx *c, double *d_xyz)
+{
+    if (!c || !d_xyz) return QMC_E_ARG;
+    QMC_CUDA(c, launch_get_positions(c, d_xyz));
+    return QMC_OK;
+}
+
+extern "C" int qmc_set_positions(qmc_ctx *c, const double *d_xyz)
+{
+    if (!c || !d_xyz) return QMC_E_ARG;
+    QMC_CUDA(c, launch_set_positions(c, d_xyz));
+    QMC_CUDA(c, launch_energy(c, nullptr, false));
+    c->t_acc0 = c->t;
+    c->have_state = true;
+    return QMC_OK;
+}
+
+extern "C" int qmc_get_pair_sums(qmc_ctx *c, double *d_S)
+{
+    if (!c || !d_S) return QMC_E_ARG;
+    c->launches += 1;
+    get_pair_sums_kernel<<<grid_wn(c, c->p.N), 128, 0, c->stream>>>(c->sv, d_S);
+    QMC_CUDA(c, cudaGetLastError());
+    return QMC_OK;
+}
+
+extern "C" int qmc_trace_decisions(qmc_ctx *c, int32_t w_begin, int32_t w_end, uint8_t *d_dec, double *d_margin,
+                                   int64_t moves_capacity)
+{
+    if (!c) return QMC_E_ARG;
+    if (d_dec && (w_begin < 0 || w_end > c->W || w_begin >= w_end || moves_capacity <= 0))
+        QMC_FAIL(c, QMC_E_ARG, "bad trace window [%d,%d) or capacity", w_begin, w_end);
+    c->trace.dec = d_dec;
+    c->trace.margin = d_dec ? d_margin : nullptr;
+    c->trace.w_begin = w_begin;
+    c->trace.w_end = w_end;
+    c->trace.capacity = moves_capacity;
+    c->trace.offset = 0;
+    return QMC_OK;
+}
+
+extern "C" int qmc_step_host(qmc_ctx *c, const double *h_xyz_in, int32_t n_sweeps, const double *steps,
+                             double *h_energy, double *h_acc, double *h_xyz_out)
+{
+    if (!c) return QMC_E_ARG;
+    const size_t W = (size_t)c->W, N = (size_t)c->p.N;
+    double *d_e = c->d_scratch, *d_a = c->d_scratch + 4 * W, *d_x = c->d_scratch + 5 * W;
+    if (h_xyz_in) {
+        QMC_CUDA(c, cudaMemcpyAsync(d_x, h_xyz_in, sizeof(double) * W * 3 * N, cudaMemcpyHostToDevice, c->stream));
+        int rc = qmc_set_positions(c, d_x);
+        if (rc != QMC_OK) return rc;
+    }
+    if (n_sweeps > 0) {
+        int rc = qmc_sweep(c, n_sweeps, steps);
+        if (rc != QMC_OK) return rc;
+    }
+    if (h_energy) {
+        int rc = qmc_local_energy(c, d_e);
+        if (rc != QMC_OK) return rc;
+        QMC_CUDA(c, cudaMemcpyAsync(h_energy, d_e, sizeof(double) * 4 * W, cudaMemcpyDeviceToHost, c->stream));
+    }
+    if (h_acc) {
+        int rc = qmc_acceptance(c, d_a);
+        if (rc != QMC_OK) return rc;
+        QMC_CUDA(c, cudaMemcpyAsync(h_acc, d_a, sizeof(double) * W, cudaMemcpyDeviceToHost, c->stream));
+    }
+    if (h_xyz_out) {
+        int rc = qmc_get_positions(c, d_x);
+        if (rc != QMC_OK) return rc;
+        QMC_CUDA(c, cudaMemcpyAsync(h_xyz_out, d_x, sizeof(double) * W * 3 * N, cudaMemcpyDeviceToHost, c->stream));
+    }
+    QMC_CUDA(c, cudaStreamSynchronize(c->stream));
+    return QMC_OK;
+}
+
+extern "C" int qmc_info(const qmc_ctx *c, qmc_info_t *out)
+{
+    if (!c || !out) return QMC_E_ARG;
+    out->W = c->W; out->N = c->p.N; out->n_groups = c->p.n_groups; out->mode = c->p.mode;
+    out->sweep_threads = c->sweep_plan.threads; out->sweep_ctas_per_sm = c->sweep_plan.ctas_per_sm;
+    out->sweep_smem_bytes = c->sweep_plan.smem_bytes; out->sweep_pairs_per_thread = c->sweep_plan.J;
+    out->energy_threads = c->energy_plan.threads; out->energy_ctas_per_sm = c->energy_plan.ctas_per_sm;
+    out->energy_smem_bytes = c->energy_plan.smem_bytes;
+    out->sm_count = c->sm_count;
+    out->t = c->t;
+    out->kernel_launches = c->launches;
+    return QMC_OK;
+}
+
+extern "C" int qmc_pipe_peak(int32_t which, void *cuda_stream, double *h_fma_per_s)
+{
+    if (!h_fma_per_s || (which != 0 && which != 1)) return QMC_E_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        snprintf(g_create_err, 512, "no CUDA device");
+        return QMC_E_CUDA;
+    }
+    void *sink = nullptr;
+    if (cudaMalloc(&sink, 64) != cudaSuccess) return QMC_E_CUDA;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = which == 0 ? 4000 : 8000;
+    const int grid = sms * 8, block = 256;
+    float best_ms = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0, st);
+        if (which == 0) fma_peak_kernel<double><<<grid, block, 0, st>>>((double *)sink, iters, 0.999999, 1e-7);
+        else            fma_peak_kernel<float><<<grid, block, 0, st>>>((float *)sink, iters, 0.999999f, 1e-7f);
+        cudaEventRecord(e1, st);
+        cudaEventSynchronize(e1);
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best_ms) best_ms = ms;
+    }
+    cudaError_t e = cudaGetLastError();
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    if (e != cudaSuccess) { snprintf(g_create_err, 512, "fma_peak_kernel: %s", cudaGetErrorString(e)); return QMC_E_CUDA; }
+    const double fmas = (double)grid * block * (double)iters * 64.0;
+    *h_fma_per_s = fmas / (best_ms * 1e-3);
+    return QMC_OK;
+}

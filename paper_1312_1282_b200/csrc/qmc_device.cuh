@@ -1,0 +1,150 @@
+// qmc_device.cuh -- device-side building blocks of the He-4 VMC hot path (sm_100a).
+//
+// Independent implementation of the definitions in DESIGN.md ("Definitions", "Randomness");
+// shares nothing with oracle/.  PAPER.md = arXiv:1312.1282.
+//
+//   pair correlation   u(r) = f(r) + f(L-r) - 2 f(L/2),  f(r) = -1/2 (b/r)^5     Eq.(8)/(9), R1
+//   written here as    u = c1 * (y^5 + z^5) + c0,  y = 1/r, z = 1/(L-r),
+//                      c1 = -b^5/2,  c0 = b^5 / h^5  (= -2 f(h)),  h = L/2
+//   minimum image      per component m = h - | h - |a-b| |   ( = min(|d|, L-|d|) for |d| <= L,
+//                      and squares to the right value for L < |d| < 3L/2 )                 l.325, R5
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace qmc {
+
+// ---------------------------------------------------------------------------------------------
+// Per-parameter-point constants (device copy, doubles; kernels narrow them for FP32C).
+// ---------------------------------------------------------------------------------------------
+struct GroupDev {
+    double L, h, h2;        // box edge, cutoff L/2, cutoff squared
+    double c1, c0;          // u = c1*(y^5+z^5) + c0
+    double b5;              // b^5 (for u', u'')
+    double step;            // proposal half-width of the current qmc_sweep call
+    double a_lat;           // FCC lattice constant L/k (R13)
+    int32_t k_lat;          // cells per edge
+    int32_t pad;
+};
+
+struct AzizDev {            // HFD-B(HE), l.131, R3
+    double eps, inv_rm, rm2, A, alpha, beta, c6, c8, c10, D, Drm;
+};
+
+// ---------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al., SC'11): 10 rounds of
+//   (c0,c1,c2,c3) <- (hi(M1*c2)^c1^k0, lo(M1*c2), hi(M0*c0)^c3^k1, lo(M0*c0)),  key += (W0,W1).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k)
+{
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+        c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
+        k.x += 0x9E3779B9u;
+        k.y += 0xBB67AE85u;
+    }
+    return c;
+}
+
+// Exact maps of a 32-bit word to (-1,1) and (0,1) (R7, R8): (2x+1)/2^32 - 1 and (2x+1)/2^33.
+__device__ __forceinline__ double word_to_pm1(uint32_t x)
+{
+    return __dadd_rn(__dmul_rn(__dadd_rn(__uint2double_rn(x), 0.5), 4.656612873077392578125e-10), -1.0);
+}
+__device__ __forceinline__ double word_to_unit(uint32_t x)
+{
+    return __dmul_rn(__dadd_rn(__uint2double_rn(x), 0.5), 2.3283064365386962890625e-10);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fast reciprocal square root / reciprocal in fp64: hardware seed (MUFU.RSQ64H / MUFU.RCP64H,
+// relative error <= ~2^-20) followed by ONE third-order correction, error ~ seed^3 < 2^-58.
+// Arguments here are always normal, positive and far from the exponent limits.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double rsqrt_pos(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double t = x * y;
+    const double e = fma(-t, y, 1.0);          // e = 1 - x y^2
+    const double p = fma(e, 0.375, 0.5);       // 1/2 + 3/8 e
+    const double q = y * e;
+    return fma(q, p, y);                       // y (1 + e/2 + 3 e^2/8)
+}
+__device__ __forceinline__ double rcp_pos(double x)
+{
+    double z;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(z) : "d"(x));
+    const double e = fma(-x, z, 1.0);          // e = 1 - x z
+    const double p = fma(e, e, e);             // e + e^2
+    return fma(z, p, z);                       // z (1 + e + e^2)
+}
+__device__ __forceinline__ float rsqrt_pos(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_pos(float x)
+{
+    float z;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(z) : "f"(x));
+    return z;
+}
+
+template <typename Real> __device__ __forceinline__ Real rabs(Real x);
+template <> __device__ __forceinline__ double rabs<double>(double x) { return fabs(x); }
+template <> __device__ __forceinline__ float rabs<float>(float x) { return fabsf(x); }
+
+// Constants of one parameter point narrowed to the arithmetic type of the mode.
+template <typename Real>
+struct PairConst {
+    Real L, h, h2, c1, c0;
+    __device__ __forceinline__ void load(const GroupDev &g)
+    {
+        L = (Real)g.L;
+        h = (Real)0.5 * L;            // exactly half of the box edge AS REPRESENTED in Real
+        h2 = h * h;
+        c1 = (Real)g.c1;
+        c0 = (Real)g.c0;
+    }
+};
+
+// Squared minimum-image distance between a and b.
+template <typename Real>
+__device__ __forceinline__ Real min_image_r2(Real ax, Real ay, Real az, Real bx, Real by, Real bz,
+                                             const PairConst<Real> &P)
+{
+    const Real mx = P.h - rabs<Real>(P.h - rabs<Real>(ax - bx));
+    const Real my = P.h - rabs<Real>(P.h - rabs<Real>(ay - by));
+    const Real mz = P.h - rabs<Real>(P.h - rabs<Real>(az - bz));
+    return fma(mz, mz, fma(my, my, mx * mx));
+}
+
+// u(r) from r^2 (> 0); 0 at and beyond the cutoff (strict '<', R2).
+template <typename Real>
+__device__ __forceinline__ Real pair_u(Real r2, const PairConst<Real> &P)
+{
+    const Real y = rsqrt_pos(r2);
+    const Real r = r2 * y;
+    const Real z = rcp_pos(P.L - r);
+    const Real y2 = y * y, z2 = z * z;
+    const Real y5 = y2 * y2 * y, z5 = z2 * z2 * z;
+    const Real u = fma(P.c1, y5 + z5, P.c0);
+    return r2 < P.h2 ? u : (Real)0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Warp / block sums.  The xor butterfly leaves the bitwise-identical total in every lane
+// (IEEE addition commutes), so every thread can take the same decision without a broadcast.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    return v;
+}
+
+}  // namespace qmc

@@ -1,0 +1,74 @@
+// qmc_internal.h -- host-side context shared by the translation units of libqmc_b200.so.
+#pragma once
+#include <cstdint>
+#include <cstdio>
+#include <vector>
+#include <cuda_runtime.h>
+
+#include "../../include/qmc.h"
+#include "qmc_device.cuh"
+
+namespace qmc {
+
+// Everything a kernel needs to find a walker's state.  Plain pointers, passed by value.
+struct StateView {
+    void     *pos;        // Real [W][3][ld]   (Real = double in FP64, float in FP32C)
+    double   *S;          // [W][ld]  running pair sums S_i = sum_{j != i} u(r_ij)
+    unsigned long long *n_acc;   // [W] accepted moves since init / set_positions
+    const int32_t *group_of;     // [W] parameter point of each walker
+    const GroupDev *groups;      // [n_groups]
+    int32_t   W, N, ld;   // ld = N rounded up to a multiple of 4 (16-byte rows)
+    uint32_t  walker_id_base;
+};
+
+struct TraceView {
+    uint8_t *dec;         // [(w_end-w_begin)][capacity] or nullptr
+    double  *margin;      // same shape or nullptr
+    int32_t  w_begin, w_end;
+    long long capacity, offset;   // offset = moves already recorded per walker
+};
+
+struct SweepPlan  { int threads, J, smem_bytes, ctas_per_sm; };
+struct EnergyPlan { int threads, smem_bytes, ctas_per_sm; };
+
+}  // namespace qmc
+
+struct qmc_ctx {
+    qmc_params p;                                  // scalar fields only; arrays below
+    std::vector<int32_t> walkers_per_group;
+    std::vector<double>  box_L, jastrow_b;
+    std::vector<qmc::GroupDev> groups;             // host mirror of d_groups
+    qmc::AzizDev aziz;
+    int32_t W = 0, ld = 0;
+    cudaStream_t stream = nullptr;
+    void *d_state = nullptr;
+    bool owns_state = false;
+    qmc::StateView sv{};
+    qmc::GroupDev *d_groups = nullptr;
+    int32_t *d_group_of = nullptr;
+    double *d_scratch = nullptr;                   // [W][4] + [W] + [W][3][N] staging for *_host calls
+    qmc::TraceView trace{};
+    qmc::SweepPlan sweep_plan{};
+    qmc::EnergyPlan energy_plan{};
+    uint64_t seed = 0;
+    uint32_t t = 0;
+    uint32_t t_acc0 = 0;                           // sweep index at which the acceptance counters were zeroed
+    bool have_state = false;
+    int sm_count = 0;
+    uint64_t launches = 0;
+    char err[512] = {0};
+};
+
+namespace qmc {
+
+// kernels' host launchers (one per translation unit); each returns a cudaError_t
+cudaError_t launch_sweep(qmc_ctx *c, int n_sweeps);
+cudaError_t launch_energy(qmc_ctx *c, double *d_out, bool energy /*false: only rebuild S_i*/);
+cudaError_t launch_init(qmc_ctx *c);
+cudaError_t launch_set_positions(qmc_ctx *c, const double *d_xyz);
+cudaError_t launch_get_positions(qmc_ctx *c, double *d_xyz);
+cudaError_t launch_acceptance(qmc_ctx *c, double *d_out);
+bool plan_sweep(qmc_ctx *c, SweepPlan *out);
+bool plan_energy(qmc_ctx *c, EnergyPlan *out);
+
+}  // namespace qmc

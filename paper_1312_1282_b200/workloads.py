@@ -177,3 +177,13 @@ def walker_shard(n_walkers: int, rank: int, world: int) -> Tuple[int, int]:
     base, rem = divmod(n_walkers, world)
     begin = rank * base + min(rank, rem)
     return begin, begin + base + (1 if rank < rem else 0)
+
+
+def shard_groups(w: Workload, begin: int, end: int) -> Tuple[List[int], int]:
+    """Walkers-per-group of the global walker range [begin, end) of `w` (walkers are numbered group by
+    group) and the global id of its first walker.  Groups outside the range get 0 walkers."""
+    lo, out = 0, []
+    for n in w.walkers_per_group:
+        out.append(max(0, min(end, lo + n) - max(begin, lo)))
+        lo += n
+    return out, begin

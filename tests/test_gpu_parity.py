@@ -1,0 +1,330 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Tolerances are BASELINE.json north_star's:
+  * fp64 mode: accept/reject decisions match move for move except where |2*Delta - log xi| < 1e-9
+    (then the chain is resynchronised by replaying the GPU's decisions in the oracle, R19);
+    committed coordinates are bit-identical; local energies agree to 1e-10 relative;
+  * fp32-coordinate mode: local energies on the same (fp32-exact) coordinates to 1e-5 relative;
+    walker-averaged energies within 3 standard errors.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1312_1282_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+AZ, DK = wl.AZIZ_HFDB_HE, wl.HBAR2_OVER_2M
+TIE = 1e-9          # north_star exemption window on 2*Delta - log(xi)
+TOL64 = 1e-10       # north_star: relative, fp64 mode
+TOL32 = 1e-5        # north_star: relative, fp32-coordinate mode
+
+
+@pytest.fixture(scope="module")
+def qmc():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1312_1282_b200 import binding, build
+    build.build()
+    binding.load_library()
+    return binding
+
+
+def make(qmc, N, W, mode, rho=wl.RHO_EQ, b=2.89, base=0, aziz=AZ, **kw):
+    L = wl.box_edge(N, rho)
+    return qmc.QMC(N, [W], [L], [b], DK, aziz, mode, walker_id_base=base, jitter=wl.JITTER, **kw), L
+
+
+def orc_sys(oracle, N, L, b=2.89, aziz=AZ):
+    return oracle.System(N, L, b, DK, aziz)
+
+
+def relerr(a, b):
+    return np.abs(a - b) / np.maximum(np.abs(b), 1e-300)
+
+
+# ------------------------------------------------------------------------------ initial state
+@pytest.mark.parametrize("N", [2, 64, 100, 256, 1952])
+def test_init_walkers_bit_identical_fp64(qmc, oracle, N):
+    q, L = make(qmc, N, 3, qmc.QMC_FP64, base=5)
+    q.init_walkers(wl.SEED)
+    x = q.get_positions().cpu().numpy()
+    ref = oracle.init_walkers(orc_sys(oracle, N, L), wl.SEED, 5, 3, wl.JITTER)
+    assert np.array_equal(x, ref)
+    S = q.pair_sums().cpu().numpy()
+    for w in range(3):
+        Sr = oracle.pair_sums(orc_sys(oracle, N, L), ref[w])
+        assert np.allclose(S[w], Sr, rtol=1e-12, atol=1e-13)
+
+
+def test_init_walkers_fp32c_is_the_rounded_lattice(qmc, oracle):
+    N = 256
+    q, L = make(qmc, N, 2, qmc.QMC_FP32C)
+    q.init_walkers(wl.SEED)
+    x = q.get_positions().cpu().numpy()
+    ref = oracle.init_walkers(orc_sys(oracle, N, L), wl.SEED, 0, 2, wl.JITTER)
+    assert np.array_equal(x, x.astype(np.float32).astype(np.float64))
+    d = x - ref
+    d -= L * np.rint(d / L)
+    assert np.abs(d).max() < 4e-6
+
+
+# ------------------------------------------------------------------------------ trajectories
+def run_and_compare_fp64(qmc, oracle, N, W, sweeps, step, rho=wl.RHO_EQ, b=2.89, base=0, split=None):
+    q, L = make(qmc, N, W, qmc.QMC_FP64, rho=rho, b=b, base=base)
+    q.init_walkers(wl.SEED)
+    dec, mar = q.trace_decisions(0, W, sweeps * N)
+    if split:
+        done = 0
+        for part in split:
+            q.sweep(part, step)
+            done += part
+        assert done == sweeps
+    else:
+        q.sweep(sweeps, step)
+    xg = q.get_positions().cpu().numpy()
+    dec, mar = dec.cpu().numpy(), mar.cpu().numpy()
+    acc = q.acceptance().cpu().numpy()
+    Sg = q.pair_sums().cpu().numpy()
+    s = orc_sys(oracle, N, L, b)
+    xo = oracle.init_walkers(s, wl.SEED, base, W, wl.JITTER)
+    # free-running oracle first: the usual case is an identical chain
+    xfree = xo.copy()
+    nacc, dec_o, mar_o = oracle.sweep(s, xfree, wl.SEED, base, 0, sweeps, step, want_trace=True)
+    exempt = 0
+    if not np.array_equal(dec_o, dec):
+        # R19: replay the GPU's decisions; every disagreement must sit inside the tie window
+        _, _, mar_o = oracle.sweep(s, xo, wl.SEED, base, 0, sweeps, step, want_trace=True, force=dec)
+        bad = (mar_o > 0) != (dec != 0)
+        assert np.all(np.abs(mar_o[bad]) < TIE), np.abs(mar_o[bad]).max()
+        exempt = int(bad.sum())
+        xfree = xo
+    assert np.array_equal(xg, xfree), "committed coordinates must be bit-identical"
+    assert np.abs(mar - mar_o).max() < TIE
+    assert np.allclose(acc, dec.sum(1) / (sweeps * N), rtol=0, atol=1e-15)
+    for w in range(min(W, 4)):                      # running sums track the definition (P12 / R17)
+        assert np.allclose(Sg[w], oracle.pair_sums(s, xg[w]), rtol=1e-11, atol=1e-11)
+    q.close()
+    return exempt, dec.mean()
+
+
+def test_trajectory_config1_full(qmc, oracle):
+    """configs[0] in full: N = 64, 64 walkers, 200 sweeps, fp64."""
+    w = wl.config(1)
+    exempt, acc = run_and_compare_fp64(qmc, oracle, w.n_atoms, w.n_walkers, w.sweeps, w.steps[0])
+    assert exempt <= 2 and 0.45 < acc < 0.6
+
+
+@pytest.mark.parametrize("N,W,sweeps", [(2, 8, 50), (33, 5, 12), (100, 6, 10), (256, 16, 8), (300, 3, 5),
+                                        (512, 4, 4), (1000, 3, 3)])
+def test_trajectory_shapes_and_ragged_tails(qmc, oracle, N, W, sweeps):
+    """several tile shapes (T = 32..256, J = 1..4) including ragged tails (N not a multiple of T)."""
+    run_and_compare_fp64(qmc, oracle, N, W, sweeps, 1.0 if N > 2 else 0.4, base=11)
+
+
+def test_trajectory_config3_size_sampled(qmc, oracle):
+    """N = 1952 in the bench launch shape (256 threads x 8 particles), a sample of walkers and sweeps."""
+    run_and_compare_fp64(qmc, oracle, 1952, 4, 2, 1.0, base=100)
+
+
+def test_split_calls_continue_the_chain(qmc, oracle):
+    """sweep(2); sweep(3); sweep(1) == sweep(6), including the trace offset (P11)."""
+    run_and_compare_fp64(qmc, oracle, 64, 4, 6, 1.0, split=(2, 3, 1))
+
+
+def test_walker_shard_reproduces_global_walkers(qmc):
+    """walker_id_base keys the stream: walkers [3,7) of a 10-walker run equal a 4-walker shard at base 3."""
+    import torch
+    for mode in (qmc.QMC_FP64, qmc.QMC_FP32C):
+        q, _ = make(qmc, 100, 10, mode)
+        q.init_walkers(7)
+        q.sweep(5, 1.0)
+        full = q.get_positions()
+        qs, _ = make(qmc, 100, 4, mode, base=3)
+        qs.init_walkers(7)
+        qs.sweep(2, 1.0)
+        qs.sweep(3, 1.0)
+        assert torch.equal(full[3:7], qs.get_positions())
+        assert torch.equal(q.acceptance()[3:7], qs.acceptance())
+
+
+def test_multi_group_config5_shape(qmc, oracle):
+    """configs[4] shape: several (rho, b) points in ONE context, per-group steps; 2 walkers per point."""
+    w = wl.config(5).truncated(2, sweeps=3)
+    q = qmc.QMC.from_workload(w)
+    q.init_walkers(w.seed)
+    dec, mar = q.trace_decisions(0, w.n_walkers, 3 * w.n_atoms)
+    q.sweep(3, w.steps)
+    xg = q.get_positions().cpu().numpy()
+    eg = q.local_energy().cpu().numpy()
+    dec = dec.cpu().numpy()
+    for g, grp in enumerate(w.groups):
+        s = oracle.System(w.n_atoms, w.box_L[g], grp.b, DK, AZ)
+        xo = oracle.init_walkers(s, w.seed, 2 * g, 2, wl.JITTER)
+        _, _, mo = oracle.sweep(s, xo, w.seed, 2 * g, 0, 3, grp.step, want_trace=True, force=dec[2 * g:2 * g + 2])
+        bad = (mo > 0) != (dec[2 * g:2 * g + 2] != 0)
+        assert np.all(np.abs(mo[bad]) < TIE)
+        assert np.array_equal(xo, xg[2 * g:2 * g + 2])
+        eo = oracle.local_energy(s, xo)[:, :4]
+        assert relerr(eg[2 * g:2 * g + 2], eo).max() < TOL64
+
+
+# ------------------------------------------------------------------------------ local energy
+@pytest.mark.parametrize("N", [2, 17, 64, 100, 256, 515, 1952])
+def test_local_energy_fp64(qmc, oracle, N):
+    W = 3
+    q, L = make(qmc, N, W, qmc.QMC_FP64)
+    xyz = np.stack([wl.liquid_configuration(N, L, 100 + N + k) for k in range(W)])
+    q.set_positions(xyz)
+    eg = q.local_energy().cpu().numpy()
+    eo = oracle.local_energy(orc_sys(oracle, N, L), xyz)
+    assert relerr(eg, eo[:, :4]).max() < TOL64, (eg, eo)
+    S = q.pair_sums().cpu().numpy()
+    for k in range(W):
+        assert np.allclose(S[k], oracle.pair_sums(orc_sys(oracle, N, L), xyz[k]), rtol=1e-12, atol=1e-13)
+
+
+@pytest.mark.parametrize("N", [64, 256, 1000, 1952])
+def test_local_energy_fp32c(qmc, oracle, N):
+    """fp32 coordinates + fp32 pair arithmetic vs the fp64 oracle on the SAME (fp32-exact) coordinates.
+    The cutoff guard (R2): a pair within fp32 rounding of L/2 may be classified differently; V jumps
+    there by V(L/2), so such configurations are skipped if the oracle reports one (never at these seeds)."""
+    W = 3
+    q, L = make(qmc, N, W, qmc.QMC_FP32C)
+    xyz = np.stack([wl.liquid_configuration(N, L, 200 + N + k, fp32_exact=True) for k in range(W)])
+    q.set_positions(xyz)
+    assert np.array_equal(q.get_positions().cpu().numpy(), xyz)
+    eg = q.local_energy().cpu().numpy()
+    eo = oracle.local_energy(orc_sys(oracle, N, L), xyz)
+    ok = eo[:, 5] > 1e-6
+    assert ok.any()
+    assert relerr(eg[ok], eo[ok, :4]).max() < TOL32, relerr(eg[ok], eo[ok, :4])
+
+
+def test_local_energy_config4_size(qmc, oracle):
+    """N = 10000 (120 KB of fp32 coordinates in shared memory), one configuration, fp32c vs oracle."""
+    N = 10000
+    q, L = make(qmc, N, 1, qmc.QMC_FP32C)
+    xyz = wl.liquid_configuration(N, L, 77, fp32_exact=True)[None]
+    q.set_positions(xyz)
+    eg = q.local_energy().cpu().numpy()
+    eo = oracle.local_energy(orc_sys(oracle, N, L), xyz)
+    assert relerr(eg, eo[:, :4]).max() < TOL32
+    # and one sweep runs at this size (1024 threads x 10 particles) leaving S consistent
+    q.sweep(1, 1.0)
+    x1 = q.get_positions().cpu().numpy()
+    S1 = q.pair_sums().cpu().numpy()[0]
+    Sr = oracle.pair_sums(orc_sys(oracle, N, L), x1[0])
+    assert np.abs(S1 - Sr).max() < 5e-5 * np.abs(Sr).max()
+    a = float(q.acceptance().cpu()[0])
+    assert 0.3 < a < 0.8
+
+
+def test_free_particles_energy_zero_acceptance_one(qmc):
+    """P2 on the GPU: b = 0 and eps = 0  =>  E_L = 0 exactly, every move accepted."""
+    az0 = (0.0,) + AZ[1:]
+    for mode in (qmc.QMC_FP64, qmc.QMC_FP32C):
+        q, _ = make(qmc, 100, 4, mode, b=0.0, aziz=az0)
+        q.init_walkers(3)
+        q.sweep(4, 1.0)
+        e = q.local_energy().cpu().numpy()
+        assert (e == 0.0).all()
+        assert (q.acceptance().cpu().numpy() == 1.0).all()
+
+
+# ------------------------------------------------------------------------------ fp32c statistics
+def test_fp32c_walker_averages_within_3_se(qmc, oracle):
+    """Walker-averaged energies of an fp32-coordinate GPU run vs an fp64 oracle run (different chains,
+    same ensemble): |difference| < 3 combined standard errors (north_star)."""
+    N, W, n_eq, n_meas = 64, 256, 100, 20
+    q, L = make(qmc, N, W, qmc.QMC_FP32C)
+    q.init_walkers(wl.SEED)
+    q.sweep(n_eq, 1.0)
+    eg = []
+    for _ in range(n_meas):
+        q.sweep(3, 1.0)
+        eg.append(q.local_energy().cpu().numpy())
+    eg = np.mean(eg, axis=0) / N                        # per-walker time averages
+    s = orc_sys(oracle, N, L)
+    xo = oracle.init_walkers(s, wl.SEED + 1, 0, W, wl.JITTER)
+    oracle.sweep(s, xo, wl.SEED + 1, 0, 0, n_eq, 1.0)
+    eo, t = [], n_eq
+    for _ in range(n_meas):
+        oracle.sweep(s, xo, wl.SEED + 1, 0, t, 3, 1.0)
+        t += 3
+        eo.append(oracle.local_energy(s, xo)[:, :4])
+    eo = np.mean(eo, axis=0) / N
+    for col in range(4):
+        diff = eg[:, col].mean() - eo[:, col].mean()
+        se = math.sqrt(eg[:, col].var(ddof=1) / W + eo[:, col].var(ddof=1) / W)
+        assert abs(diff) < 3 * se, (col, diff, se)
+    ag = float(q.acceptance().cpu().mean())
+    assert 0.45 < ag < 0.6
+
+
+def test_fp32c_pair_sums_do_not_drift(qmc, oracle):
+    """Running S_i after 60 fp32c sweeps still equal the from-scratch sums to fp32 accuracy, and the
+    energy pass rebuilds them (R17)."""
+    N = 256
+    q, L = make(qmc, N, 2, qmc.QMC_FP32C)
+    q.init_walkers(9)
+    q.sweep(60, 1.0)
+    x = q.get_positions().cpu().numpy()
+    S = q.pair_sums().cpu().numpy()
+    s = orc_sys(oracle, N, L)
+    for w in range(2):
+        Sr = oracle.pair_sums(s, x[w])
+        assert np.abs(S[w] - Sr).max() < 2e-5 * np.abs(Sr).max()
+    q.local_energy()
+    S2 = q.pair_sums().cpu().numpy()
+    for w in range(2):
+        Sr = oracle.pair_sums(s, x[w])
+        assert np.abs(S2[w] - Sr).max() < 2e-6 * np.abs(Sr).max()
+
+
+# ------------------------------------------------------------------------------ boundary behaviour
+def test_error_codes(qmc):
+    with pytest.raises(qmc.QmcError) as e:
+        make(qmc, 10000, 1, qmc.QMC_FP64)                   # 240 KB of fp64 coordinates: R-capacity
+    assert e.value.code == qmc.QMC_E_CAPACITY
+    q, L = make(qmc, 64, 2, qmc.QMC_FP64)
+    with pytest.raises(qmc.QmcError) as e:
+        q.sweep(1, 1.0)                                     # no state yet
+    assert e.value.code == qmc.QMC_E_STATE
+    q.init_walkers(1)
+    with pytest.raises(qmc.QmcError) as e:
+        q.sweep(1, L)                                       # step >= L/2
+    assert e.value.code == qmc.QMC_E_ARG
+    q.sweep(0, 1.0)                                         # no-op
+    assert q.info()["t"] == 0
+
+
+def test_step_host_equals_device_calls(qmc):
+    """qmc_step_host (host buffers in/out) == set_positions + sweep + local_energy + acceptance."""
+    import torch
+    N, W = 100, 6
+    for mode in (qmc.QMC_FP64, qmc.QMC_FP32C):
+        q, L = make(qmc, N, W, mode, library_owns_state=True)
+        xyz = np.stack([wl.liquid_configuration(N, L, 300 + k, fp32_exact=True) for k in range(W)])
+        h_in = torch.from_numpy(xyz).pin_memory()
+        h_e = torch.empty((W, 4), dtype=torch.float64).pin_memory()
+        h_a = torch.empty((W,), dtype=torch.float64).pin_memory()
+        h_x = torch.empty((W, 3, N), dtype=torch.float64).pin_memory()
+        q.set_seed(5, 0)
+        q.step_host(3, 1.0, h_in, h_e, h_a, h_x)
+        q2, _ = make(qmc, N, W, mode)
+        q2.set_seed(5, 0)
+        q2.set_positions(xyz)
+        q2.sweep(3, 1.0)
+        assert torch.equal(q2.local_energy().cpu(), h_e)
+        assert torch.equal(q2.acceptance().cpu(), h_a)
+        assert torch.equal(q2.get_positions().cpu(), h_x)
+
+
+def test_pipe_peak_microbenchmark_is_plausible(qmc):
+    f64 = qmc.pipe_peak(0)
+    f32 = qmc.pipe_peak(1)
+    # 148 SMs x 64 (fp64) / 128 (fp32) lanes x ~1.9 GHz, allow wide margins
+    assert 8e12 < f64 < 2.2e13, f64
+    assert 1.6e13 < f32 < 4.4e13, f32
