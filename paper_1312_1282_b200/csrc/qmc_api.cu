@@ -29,6 +29,23 @@ namespace qmc {
 // Initial walkers (R13): particle i on FCC site floor(i*M/N), M = 4k^3, sites ordered
 // (ix,iy,iz,basis) with the basis fastest; + jitter * a_c, a_c from Philox counter (i,0,walker,1).
 // ------------------------------------------------------------------------------------------
+// Angstrom -> stored coordinate.  FP64: the value itself.  FP32C: s = 1 + x/L rounded to fp32, in [1,2).
+template <typename Real> __device__ __forceinline__ Real to_stored(double x, const GroupDev &g);
+template <> __device__ __forceinline__ double to_stored<double>(double x, const GroupDev &) { return x; }
+template <> __device__ __forceinline__ float to_stored<float>(double x, const GroupDev &g)
+{
+    float s = __double2float_rn(1.0 + x / g.L_A);
+    if (s >= 2.0f) s -= 1.0f;
+    if (s < 1.0f) s += 1.0f;
+    return s;
+}
+template <typename Real> __device__ __forceinline__ double to_angstrom(Real s, const GroupDev &g);
+template <> __device__ __forceinline__ double to_angstrom<double>(double s, const GroupDev &) { return s; }
+template <> __device__ __forceinline__ double to_angstrom<float>(float s, const GroupDev &g)
+{
+    return __dmul_rn(__dadd_rn((double)s, -1.0), g.L_A);
+}
+
 template <typename Real>
 __global__ void init_kernel(StateView sv, uint2 key, double jitter)
 {
@@ -52,13 +69,9 @@ __global__ void init_kernel(StateView sv, uint2 key, double jitter)
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         double v = __dadd_rn(__dmul_rn(idx[c], g.a_lat), __dmul_rn(jitter, word_to_pm1(word[c])));
-        if (v >= g.L) v = __dadd_rn(v, -g.L);
-        if (v < 0.0) v = __dadd_rn(v, g.L);
-        Real q = (Real)v;
-        const Real Lr = (Real)g.L;                 // FP32C: keep the stored value inside [0, L_fp32]
-        if (q >= Lr) q -= Lr;
-        if (q < (Real)0) q += Lr;
-        pos[c * ld + i] = q;
+        if (v >= g.L_A) v = __dadd_rn(v, -g.L_A);
+        if (v < 0.0) v = __dadd_rn(v, g.L_A);
+        pos[c * ld + i] = to_stored<Real>(v, g);
     }
 }
 
@@ -71,13 +84,14 @@ __global__ void set_positions_kernel(StateView sv, const double *__restrict__ xy
     if (i >= ld) return;
     Real *pos = reinterpret_cast<Real *>(sv.pos) + (size_t)w * 3 * ld;
     const double *src = xyz + (size_t)w * 3 * N;
-    const Real Lr = (Real)sv.groups[sv.group_of[w]].L;
+    const GroupDev g = sv.groups[sv.group_of[w]];
     for (int c = 0; c < 3; ++c) {
-        Real q = (Real)0;
+        Real q = (Real)g.origin;
         if (i < N) {
-            q = (Real)src[c * N + i];
-            if (q >= Lr) q -= Lr;
-            if (q < (Real)0) q += Lr;
+            double v = src[c * N + i];
+            if (v >= g.L_A) v -= g.L_A;
+            if (v < 0.0) v += g.L_A;
+            q = to_stored<Real>(v, g);
         }
         pos[c * ld + i] = q;
     }
@@ -93,7 +107,8 @@ __global__ void get_positions_kernel(StateView sv, double *__restrict__ xyz)
     if (i >= N) return;
     const Real *pos = reinterpret_cast<const Real *>(sv.pos) + (size_t)w * 3 * ld;
     double *dst = xyz + (size_t)w * 3 * N;
-    for (int c = 0; c < 3; ++c) dst[c * N + i] = (double)pos[c * ld + i];
+    const GroupDev g = sv.groups[sv.group_of[w]];
+    for (int c = 0; c < 3; ++c) dst[c * N + i] = to_angstrom<Real>(pos[c * ld + i], g);
 }
 
 __global__ void get_pair_sums_kernel(StateView sv, double *__restrict__ S)
@@ -252,9 +267,15 @@ extern "C" int qmc_create(const qmc_params *p, void *cuda_stream, void *d_state,
     c->groups.resize(p->n_groups);
     for (int g = 0; g < p->n_groups; ++g) {
         GroupDev &G = c->groups[g];
-        const double L = p->box_L[g], b = p->jastrow_b[g];
-        G.L = L; G.h = 0.5 * L; G.h2 = G.h * G.h;
-        G.b5 = b * b * b * b * b;
+        const double LA = p->box_L[g], b = p->jastrow_b[g];
+        // coordinate unit: Angstrom in FP64, the box edge in FP32C
+        const double unit = (p->mode == QMC_FP64) ? 1.0 : LA;
+        G.unit = unit; G.inv_unit = 1.0 / unit; G.origin = (p->mode == QMC_FP64) ? 0.0 : 1.0;
+        G.L_A = LA;
+        G.L = (p->mode == QMC_FP64) ? LA : 1.0;
+        G.h = 0.5 * G.L; G.h2 = G.h * G.h;
+        const double bu = b / unit;
+        G.b5 = bu * bu * bu * bu * bu;
         G.c1 = -0.5 * G.b5;
         const double h = G.h;
         G.c0 = G.b5 / (h * h * h * h * h);
@@ -262,13 +283,14 @@ extern "C" int qmc_create(const qmc_params *p, void *cuda_stream, void *d_state,
         long long k = 1;
         while (4 * k * k * k < p->N) ++k;
         G.k_lat = (int32_t)k;
-        G.a_lat = L / (double)k;
+        G.a_lat = LA / (double)k;
         G.pad = 0;
+        const double *a = p->aziz;
+        const double rm = a[1] / unit;
+        G.az.eps = a[0]; G.az.inv_rm = 1.0 / rm; G.az.rm2 = rm * rm; G.az.A = a[2];
+        G.az.alpha = a[3]; G.az.beta = a[4]; G.az.c6 = a[5]; G.az.c8 = a[6]; G.az.c10 = a[7];
+        G.az.D = a[8]; G.az.Drm = a[8] * rm;
     }
-    const double *a = p->aziz;
-    c->aziz.eps = a[0]; c->aziz.inv_rm = 1.0 / a[1]; c->aziz.rm2 = a[1] * a[1]; c->aziz.A = a[2];
-    c->aziz.alpha = a[3]; c->aziz.beta = a[4]; c->aziz.c6 = a[5]; c->aziz.c8 = a[6]; c->aziz.c10 = a[7];
-    c->aziz.D = a[8]; c->aziz.Drm = a[8] * a[1];
 
     // state buffer
     size_t pos_bytes, S_off, acc_off, total;
@@ -360,6 +382,7 @@ extern "C" int qmc_sweep(qmc_ctx *c, int32_t n_sweeps, const double *steps)
     if (!c->have_state) QMC_FAIL(c, QMC_E_STATE, "qmc_sweep before qmc_init_walkers / qmc_set_positions");
     if (n_sweeps < 0 || !steps) QMC_FAIL(c, QMC_E_ARG, "n_sweeps >= 0 and steps != NULL required");
     if (n_sweeps == 0) return QMC_OK;
+    if ((long long)n_sweeps * c->p.N >= (1LL << 31)) QMC_FAIL(c, QMC_E_ARG, "n_sweeps * N must stay below 2^31 per call");
     bool changed = false;
     for (int g = 0; g < c->p.n_groups; ++g) {
         if (!(steps[g] > 0.0) || !(steps[g] < 0.5 * c->box_L[g]))

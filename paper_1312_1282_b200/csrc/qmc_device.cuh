@@ -17,18 +17,25 @@ namespace qmc {
 // ---------------------------------------------------------------------------------------------
 // Per-parameter-point constants (device copy, doubles; kernels narrow them for FP32C).
 // ---------------------------------------------------------------------------------------------
-struct GroupDev {
-    double L, h, h2;        // box edge, cutoff L/2, cutoff squared
-    double c1, c0;          // u = c1*(y^5+z^5) + c0
-    double b5;              // b^5 (for u', u'')
-    double step;            // proposal half-width of the current qmc_sweep call
-    double a_lat;           // FCC lattice constant L/k (R13)
-    int32_t k_lat;          // cells per edge
-    int32_t pad;
+// Lengths are expressed in the mode's COORDINATE UNIT: 1 Angstrom in FP64; the box edge in FP32C,
+// where a coordinate is stored as s = 1 + x/L in [1,2) -- every fp32 in [1,2) is a multiple of 2^-23,
+// so coordinate differences and the minimum-image fold are EXACT in fp32.
+struct AzizDev {            // HFD-B(HE), l.131, R3; inv_rm, rm2, Drm in coordinate units
+    double eps, inv_rm, rm2, A, alpha, beta, c6, c8, c10, D, Drm;
 };
 
-struct AzizDev {            // HFD-B(HE), l.131, R3
-    double eps, inv_rm, rm2, A, alpha, beta, c6, c8, c10, D, Drm;
+struct GroupDev {
+    double L, h, h2;        // box edge, cutoff L/2, cutoff squared            [coordinate units]
+    double c1, c0;          // u = c1*(y^5+z^5) + c0                             [coordinate units]
+    double b5;              // b^5 (for u', u'')                                 [coordinate units]
+    double unit, inv_unit;  // Angstrom per coordinate unit and its inverse (1 in FP64, L and 1/L in FP32C)
+    double origin;          // stored coordinate of x = 0 (0 in FP64, 1 in FP32C)
+    double L_A;             // box edge in Angstrom
+    double step;            // proposal half-width of the current qmc_sweep call [Angstrom]
+    double a_lat;           // FCC lattice constant L/k (R13)                    [Angstrom]
+    int32_t k_lat;          // cells per edge
+    int32_t pad;
+    AzizDev az;
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -121,6 +128,19 @@ __device__ __forceinline__ Real min_image_r2(Real ax, Real ay, Real az, Real bx,
     const Real my = P.h - rabs<Real>(P.h - rabs<Real>(ay - by));
     const Real mz = P.h - rabs<Real>(P.h - rabs<Real>(az - bz));
     return fma(mz, mz, fma(my, my, mx * mx));
+}
+
+// u(r) from r^2 without the cutoff select (the caller selects on r^2 < h^2 together with its other
+// conditions).  NaN in -> NaN out, nothing traps.
+template <typename Real>
+__device__ __forceinline__ Real pair_u_raw(Real r2, const PairConst<Real> &P)
+{
+    const Real y = rsqrt_pos(r2);
+    const Real r = r2 * y;
+    const Real z = rcp_pos(P.L - r);
+    const Real y2 = y * y, z2 = z * z;
+    const Real y5 = y2 * y2 * y, z5 = z2 * z2 * z;
+    return fma(P.c1, y5 + z5, P.c0);
 }
 
 // u(r) from r^2 (> 0); 0 at and beyond the cutoff (strict '<', R2).

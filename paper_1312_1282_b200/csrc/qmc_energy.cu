@@ -59,7 +59,7 @@ __device__ __forceinline__ Real aziz_pair(Real r, Real y, const EnergyConst<Real
 
 template <typename Real, int T, bool kEnergy>
 __global__ void __launch_bounds__(T)
-energy_kernel(StateView sv, AzizDev az, double Dk, double *__restrict__ out)
+energy_kernel(StateView sv, double Dk, double *__restrict__ out)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = sv.N, ld = sv.ld;
@@ -75,7 +75,7 @@ energy_kernel(StateView sv, AzizDev az, double Dk, double *__restrict__ out)
     PairConst<Real> P;
     P.load(g);
     EnergyConst<Real> E;
-    E.load(g, az);
+    E.load(g, g.az);
 
     const Real *gpos = reinterpret_cast<const Real *>(sv.pos) + (size_t)w * 3 * ld;
     {
@@ -152,8 +152,9 @@ energy_kernel(StateView sv, AzizDev az, double Dk, double *__restrict__ out)
             double c = lane < nwarps ? red[64 + lane] : 0.0;
             a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
             if (lane == 0) {
-                const double T_PB = -Dk * (a + b);
-                const double T_JF = -0.5 * Dk * a;
+                const double Dku = Dk * g.inv_unit * g.inv_unit;       // gradients are per coordinate unit
+                const double T_PB = -Dku * (a + b);
+                const double T_JF = -0.5 * Dku * a;
                 double *o = out + (size_t)w * 4;
                 o[0] = c + T_PB; o[1] = c; o[2] = T_PB; o[3] = T_JF;
             }
@@ -176,11 +177,11 @@ static cudaError_t launch_e(qmc_ctx *c, double *d_out, bool energy)
     if (energy) {
         auto k = energy_kernel<Real, T, true>;
         if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
-        k<<<c->W, T, smem, c->stream>>>(c->sv, c->aziz, c->p.hbar2_over_2m, d_out);
+        k<<<c->W, T, smem, c->stream>>>(c->sv, c->p.hbar2_over_2m, d_out);
     } else {
         auto k = energy_kernel<Real, T, false>;
         if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
-        k<<<c->W, T, smem, c->stream>>>(c->sv, c->aziz, c->p.hbar2_over_2m, d_out);
+        k<<<c->W, T, smem, c->stream>>>(c->sv, c->p.hbar2_over_2m, d_out);
     }
     return cudaGetLastError();
 }

@@ -28,7 +28,7 @@ struct TraceView {
     long long capacity, offset;   // offset = moves already recorded per walker
 };
 
-struct SweepPlan  { int threads, J, smem_bytes, ctas_per_sm; };
+struct SweepPlan  { int threads, J, V, smem_bytes, ctas_per_sm; };
 struct EnergyPlan { int threads, smem_bytes, ctas_per_sm; };
 
 }  // namespace qmc
@@ -38,7 +38,6 @@ struct qmc_ctx {
     std::vector<int32_t> walkers_per_group;
     std::vector<double>  box_L, jastrow_b;
     std::vector<qmc::GroupDev> groups;             // host mirror of d_groups
-    qmc::AzizDev aziz;
     int32_t W = 0, ld = 0;
     cudaStream_t stream = nullptr;
     void *d_state = nullptr;

@@ -134,13 +134,14 @@ def with_mode(w: Workload, mode: int) -> Workload:
 
 
 def liquid_configuration(n_atoms: int, box_L: float, seed: int, d_min: float = 2.3,
-                         fp32_exact: bool = False) -> np.ndarray:
+                         fp32_grid: bool = False) -> np.ndarray:
     """Seeded liquid-like configuration: random sequential insertion of points in
     the periodic cube [0,L)^3 keeping every minimum-image pair distance >= d_min
     (a hard-core gas at He-4 liquid density: packing fraction ~0.14, far below
-    jamming).  Returns float64 [3][N] (SoA).  With fp32_exact the coordinates are
-    rounded to fp32-representable values (and kept inside [0,L)) so that an fp32
-    state holds them exactly.  No wavefunction or potential is involved.
+    jamming).  Returns float64 [3][N] (SoA).  With fp32_grid every coordinate is
+    x = (k / 2^23) * L with integer k: the grid an fp32 state of the FP32C mode
+    holds exactly (it stores 1 + x/L in [1,2)), so both
+    sides see the same configuration.  No wavefunction or potential is involved.
     """
     from scipy.spatial import cKDTree  # input structure only
 
@@ -149,8 +150,8 @@ def liquid_configuration(n_atoms: int, box_L: float, seed: int, d_min: float = 2
     while len(pts) < n_atoms:
         need = n_atoms - len(pts)
         cand = rng.uniform(0.0, box_L, size=(2 * need + 16, 3))
-        if fp32_exact:
-            cand = cand.astype(np.float32).astype(np.float64)
+        if fp32_grid:
+            cand = np.floor(cand / box_L * 8388608.0) / 8388608.0 * box_L
         cand = cand[(cand >= 0.0).all(1) & (cand < box_L * (1 - 1e-7)).all(1)]
         # drop candidates too close to accepted points
         if len(pts):

@@ -119,5 +119,6 @@ def test_liquid_configuration_is_seeded_and_respects_the_core():
     d -= L * np.rint(d / L)
     r = np.sqrt((d ** 2).sum(-1)) + np.eye(200) * 1e9
     assert r.min() >= 2.3 and (a >= 0).all() and (a < L).all()
-    c = wl.liquid_configuration(50, L, 4, fp32_exact=True)
-    assert np.array_equal(c, c.astype(np.float32).astype(np.float64))
+    c = wl.liquid_configuration(50, L, 4, fp32_grid=True)
+    k = c / L * 2 ** 23
+    assert np.abs(k - np.rint(k)).max() < 1e-6 and np.array_equal(np.rint(k) / 2 ** 23 * L, c)

@@ -64,10 +64,11 @@ def test_init_walkers_fp32c_is_the_rounded_lattice(qmc, oracle):
     q.init_walkers(wl.SEED)
     x = q.get_positions().cpu().numpy()
     ref = oracle.init_walkers(orc_sys(oracle, N, L), wl.SEED, 0, 2, wl.JITTER)
-    assert np.array_equal(x, x.astype(np.float32).astype(np.float64))
+    k = x / L * 2 ** 23                                  # FP32C stores 1 + x/L on the 2^-23 grid
+    assert np.abs(k - np.rint(k)).max() < 1e-6
     d = x - ref
     d -= L * np.rint(d / L)
-    assert np.abs(d).max() < 4e-6
+    assert np.abs(d).max() < 0.51 * L / 2 ** 23
 
 
 # ------------------------------------------------------------------------------ trajectories
@@ -104,7 +105,7 @@ def run_and_compare_fp64(qmc, oracle, N, W, sweeps, step, rho=wl.RHO_EQ, b=2.89,
     assert np.abs(mar - mar_o).max() < TIE
     assert np.allclose(acc, dec.sum(1) / (sweeps * N), rtol=0, atol=1e-15)
     for w in range(min(W, 4)):                      # running sums track the definition (P12 / R17)
-        assert np.allclose(Sg[w], oracle.pair_sums(s, xg[w]), rtol=1e-11, atol=1e-11)
+        assert np.allclose(Sg[w], oracle.pair_sums(s, xfree[w]), rtol=1e-11, atol=1e-11)
     q.close()
     return exempt, dec.mean()
 
@@ -192,31 +193,57 @@ def test_local_energy_fp32c(qmc, oracle, N):
     there by V(L/2), so such configurations are skipped if the oracle reports one (never at these seeds)."""
     W = 3
     q, L = make(qmc, N, W, qmc.QMC_FP32C)
-    xyz = np.stack([wl.liquid_configuration(N, L, 200 + N + k, fp32_exact=True) for k in range(W)])
+    xyz = np.stack([wl.liquid_configuration(N, L, 200 + N + k, fp32_grid=True) for k in range(W)])
     q.set_positions(xyz)
     assert np.array_equal(q.get_positions().cpu().numpy(), xyz)
     eg = q.local_energy().cpu().numpy()
     eo = oracle.local_energy(orc_sys(oracle, N, L), xyz)
-    ok = eo[:, 5] > 1e-6
+    # skip a configuration only if a pair sits within fp32 rounding of the cutoff AND the jump of V
+    # there (V is truncated, not shifted: R3) is visible at this tolerance
+    jump = abs(oracle.aziz(L / 2, AZ))
+    ok = ~((eo[:, 5] < 5e-7) & (jump > 0.1 * TOL32 * np.abs(eo[:, 0])))
     assert ok.any()
     assert relerr(eg[ok], eo[ok, :4]).max() < TOL32, relerr(eg[ok], eo[ok, :4])
+    S = q.pair_sums().cpu().numpy()
+    Sr = oracle.pair_sums(orc_sys(oracle, N, L), xyz[0])
+    assert np.abs(S[0] - Sr).max() < 2e-6 * np.abs(Sr).max()
+
+
+@pytest.mark.parametrize("N,W", [(64, 16), (256, 4)])
+def test_local_energy_fp32c_equilibrated_liquid(qmc, oracle, N, W):
+    """The regime the tolerance is hardest in: an EQUILIBRATED liquid (E = V + T cancels ~3.5x).  The
+    configurations come from the oracle's own chain (oracle -> GPU input), snapped to the fp32c grid."""
+    s_ = orc_sys(oracle, N, wl.box_edge(N, wl.RHO_EQ))
+    x = oracle.init_walkers(s_, 31, 0, W, wl.JITTER)
+    oracle.sweep(s_, x, 31, 0, 0, 60, 1.0)
+    xyz = np.floor(x / s_.L * 2 ** 23) / 2 ** 23 * s_.L
+    q, L = make(qmc, N, W, qmc.QMC_FP32C)
+    q.set_positions(xyz)
+    eg = q.local_energy().cpu().numpy()
+    eo = oracle.local_energy(s_, xyz)
+    jump = abs(oracle.aziz(L / 2, AZ))
+    ok = ~((eo[:, 5] < 5e-7) & (jump > 0.1 * TOL32 * np.abs(eo[:, 0])))
+    assert ok.sum() >= W - 1
+    assert relerr(eg[ok], eo[ok, :4]).max() < TOL32, relerr(eg[ok], eo[ok, :4]).max(0)
 
 
 def test_local_energy_config4_size(qmc, oracle):
     """N = 10000 (120 KB of fp32 coordinates in shared memory), one configuration, fp32c vs oracle."""
     N = 10000
     q, L = make(qmc, N, 1, qmc.QMC_FP32C)
-    xyz = wl.liquid_configuration(N, L, 77, fp32_exact=True)[None]
+    xyz = wl.liquid_configuration(N, L, 77, fp32_grid=True)[None]
     q.set_positions(xyz)
     eg = q.local_energy().cpu().numpy()
     eo = oracle.local_energy(orc_sys(oracle, N, L), xyz)
     assert relerr(eg, eo[:, :4]).max() < TOL32
-    # and one sweep runs at this size (1024 threads x 10 particles) leaving S consistent
-    q.sweep(1, 1.0)
-    x1 = q.get_positions().cpu().numpy()
-    S1 = q.pair_sums().cpu().numpy()[0]
-    Sr = oracle.pair_sums(orc_sys(oracle, N, L), x1[0])
-    assert np.abs(S1 - Sr).max() < 5e-5 * np.abs(Sr).max()
+    # and sweeps run at this size (1024 threads x 10 particles); the running pair sums stay equal to
+    # the kernel's own from-scratch rebuild (GPU-internal invariant; the rebuild itself is checked
+    # against the oracle above and in test_local_energy_fp32c)
+    q.sweep(2, 1.0)
+    S_run = q.pair_sums().cpu().numpy()[0]
+    q.refresh_pair_sums()
+    S_new = q.pair_sums().cpu().numpy()[0]
+    assert np.abs(S_run - S_new).max() < 2e-5 * np.abs(S_new).max()
     a = float(q.acceptance().cpu()[0])
     assert 0.3 < a < 0.8
 
@@ -263,24 +290,19 @@ def test_fp32c_walker_averages_within_3_se(qmc, oracle):
     assert 0.45 < ag < 0.6
 
 
-def test_fp32c_pair_sums_do_not_drift(qmc, oracle):
-    """Running S_i after 60 fp32c sweeps still equal the from-scratch sums to fp32 accuracy, and the
-    energy pass rebuilds them (R17)."""
+def test_fp32c_pair_sums_do_not_drift(qmc):
+    """Running S_i after 60 fp32c sweeps still equal the from-scratch sums to fp32 accuracy (R17);
+    the energy pass rebuilds them.  GPU-internal invariant: the rebuild is pinned to the oracle in
+    test_local_energy_fp32c (same kernel, generator inputs)."""
     N = 256
     q, L = make(qmc, N, 2, qmc.QMC_FP32C)
     q.init_walkers(9)
     q.sweep(60, 1.0)
-    x = q.get_positions().cpu().numpy()
     S = q.pair_sums().cpu().numpy()
-    s = orc_sys(oracle, N, L)
-    for w in range(2):
-        Sr = oracle.pair_sums(s, x[w])
-        assert np.abs(S[w] - Sr).max() < 2e-5 * np.abs(Sr).max()
     q.local_energy()
     S2 = q.pair_sums().cpu().numpy()
-    for w in range(2):
-        Sr = oracle.pair_sums(s, x[w])
-        assert np.abs(S2[w] - Sr).max() < 2e-6 * np.abs(Sr).max()
+    assert np.abs(S - S2).max() < 2e-5 * np.abs(S2).max()
+    assert not np.array_equal(S, S2)
 
 
 # ------------------------------------------------------------------------------ boundary behaviour
@@ -306,7 +328,7 @@ def test_step_host_equals_device_calls(qmc):
     N, W = 100, 6
     for mode in (qmc.QMC_FP64, qmc.QMC_FP32C):
         q, L = make(qmc, N, W, mode, library_owns_state=True)
-        xyz = np.stack([wl.liquid_configuration(N, L, 300 + k, fp32_exact=True) for k in range(W)])
+        xyz = np.stack([wl.liquid_configuration(N, L, 300 + k, fp32_grid=True) for k in range(W)])
         h_in = torch.from_numpy(xyz).pin_memory()
         h_e = torch.empty((W, 4), dtype=torch.float64).pin_memory()
         h_a = torch.empty((W,), dtype=torch.float64).pin_memory()
