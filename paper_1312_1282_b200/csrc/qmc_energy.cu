@@ -18,18 +18,48 @@ namespace qmc {
 
 constexpr int kFlush = 16;
 
-template <typename Real> __device__ __forceinline__ Real rexp(Real x);
-template <> __device__ __forceinline__ double rexp<double>(double x) { return exp(x); }
-template <> __device__ __forceinline__ float rexp<float>(float x) { return expf(x); }
+// Constants of the energy pass in the arithmetic type of the mode.
+//
+// FP64: the potential as DESIGN.md §2 writes it.
+// FP32C: every constant that multiplies into the steep repulsive exponential or the dispersion sum is
+// either folded (in fp64, on load) into ONE rounded coefficient or carried as a hi + lo pair, so that no
+// fp32 rounding of a CONSTANT adds a systematic relative error to every pair (the box-unit value of r_m
+// is an arbitrary real number; its fp32 rounding alone would shift the exponent argument by ~6e-7):
+//   rep  = eps A exp(a1 r + a2 r^2),  a1 = -alpha / r_m,  a2 = beta / r_m^2   (hi + lo)
+//   disp = w^3 (k6 + w (k8 + w k10)),  w = fl(r_m^2) y^2,  k_n = eps c_n (r_m^2 / fl(r_m^2))^(n/2)
+//   F    = exp(-(D r_m y - 1)^2)                                                  (D r_m hi + lo)
+template <typename Real> struct EnergyConst;
 
-template <typename Real>
-struct EnergyConst {
-    Real b5, eps, inv_rm, rm2, A, alpha, beta, c6, c8, c10, D, Drm;
+template <> struct EnergyConst<double> {
+    double b5, eps, inv_rm, rm2, A, alpha, beta, c6, c8, c10, D, Drm;
     __device__ __forceinline__ void load(const GroupDev &g, const AzizDev &a)
     {
-        b5 = (Real)g.b5; eps = (Real)a.eps; inv_rm = (Real)a.inv_rm; rm2 = (Real)a.rm2; A = (Real)a.A;
-        alpha = (Real)a.alpha; beta = (Real)a.beta; c6 = (Real)a.c6; c8 = (Real)a.c8; c10 = (Real)a.c10;
-        D = (Real)a.D; Drm = (Real)a.Drm;
+        b5 = g.b5; eps = a.eps; inv_rm = a.inv_rm; rm2 = a.rm2; A = a.A;
+        alpha = a.alpha; beta = a.beta; c6 = a.c6; c8 = a.c8; c10 = a.c10;
+        D = a.D; Drm = a.Drm;
+    }
+};
+
+__device__ __forceinline__ void split_hi_lo(double v, float &hi, float &lo)
+{
+    hi = __double2float_rn(v);
+    lo = __double2float_rn(v - (double)hi);
+}
+
+template <> struct EnergyConst<float> {
+    float b5, a1h, a1l, a2h, a2l, epsA, rm2, k6, k8, k10, Drm, Drml;
+    __device__ __forceinline__ void load(const GroupDev &g, const AzizDev &a)
+    {
+        b5 = (float)g.b5;
+        split_hi_lo(-a.alpha * a.inv_rm, a1h, a1l);
+        split_hi_lo(a.beta * a.inv_rm * a.inv_rm, a2h, a2l);
+        epsA = (float)(a.eps * a.A);
+        rm2 = (float)a.rm2;
+        const double q = a.rm2 / (double)rm2;             // 1 + rounding error of fl(r_m^2)
+        k6 = (float)(a.eps * a.c6 * q * q * q);
+        k8 = (float)(a.eps * a.c8 * q * q * q * q);
+        k10 = (float)(a.eps * a.c10 * q * q * q * q * q);
+        split_hi_lo(a.Drm, Drm, Drml);
     }
 };
 
@@ -41,20 +71,43 @@ __device__ __forceinline__ Real min_image_signed(Real d, const PairConst<Real> &
     return d - shift;
 }
 
-// HFD-B(HE) in K from r and y = 1/r.
-template <typename Real>
-__device__ __forceinline__ Real aziz_pair(Real r, Real y, const EnergyConst<Real> &E)
+// HFD-B(HE) in K from r^2, r and y = 1/r.
+__device__ __forceinline__ double aziz_pair(double, double r, double y, const EnergyConst<double> &E)
 {
-    const Real x = r * E.inv_rm;
-    const Real w = E.rm2 * y * y;                               // 1/x^2
-    const Real disp = w * w * w * fma(w, fma(w, E.c10, E.c8), E.c6);
-    Real F = (Real)1;
+    const double x = r * E.inv_rm;
+    const double w = E.rm2 * y * y;                             // 1/x^2
+    const double disp = w * w * w * fma(w, fma(w, E.c10, E.c8), E.c6);
+    double F = 1.0;
     if (x < E.D) {
-        const Real t = E.Drm * y - (Real)1;                     // D/x - 1
-        F = rexp<Real>(-t * t);
+        const double t = E.Drm * y - 1.0;                       // D/x - 1
+        F = exp(-t * t);
     }
-    const Real rep = E.A * rexp<Real>(x * fma(E.beta, x, -E.alpha));
+    const double rep = E.A * exp(x * fma(E.beta, x, -E.alpha));
     return E.eps * (rep - F * disp);
+}
+
+// FP32C: y is first refined by one Newton step (the hardware rsqrt seed is good to ~2^-22, and the
+// repulsive exponential amplifies a relative error of r ~11x); the exponent argument is carried as
+// hi + lo, exp(hi + lo) = exp(hi) (1 + lo).
+__device__ __forceinline__ float aziz_pair(float r2, float, float y0, const EnergyConst<float> &E)
+{
+    const float e = fmaf(-r2 * y0, y0, 1.0f);
+    const float y = fmaf(0.5f * y0, e, y0);
+    const float r = r2 * y;
+    const float w = E.rm2 * y * y;
+    const float disp = w * w * w * fmaf(w, fmaf(w, E.k10, E.k8), E.k6);
+    float F = 1.0f;
+    if (r < E.Drm) {
+        const float t = fmaf(E.Drml, y, fmaf(E.Drm, y, -1.0f));
+        F = expf(-t * t);
+    }
+    const float t1 = fmaf(E.a2h, r, E.a1h);
+    const float ah = r * t1;
+    float al = fmaf(r, t1, -ah);                                // exact residual of the product
+    al = fmaf(r, fmaf(E.a2l, r, E.a1l), al);
+    const float ex = E.epsA * expf(ah);
+    const float rep = fmaf(ex, al, ex);
+    return rep - F * disp;
 }
 
 template <typename Real, int T, bool kEnergy>
@@ -123,7 +176,7 @@ energy_kernel(StateView sv, double Dk, double *__restrict__ out)
                     plam += in ? lt : (Real)0;
                     const bool needV = in && (j > ic);
                     if (__any_sync(0xffffffffu, needV)) {
-                        const Real vp = aziz_pair<Real>(r, yy, E);
+                        const Real vp = aziz_pair(r2, r, yy, E);
                         pv += needV ? vp : (Real)0;
                     }
                 }

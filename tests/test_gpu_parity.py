@@ -44,6 +44,15 @@ def relerr(a, b):
     return np.abs(a - b) / np.maximum(np.abs(b), 1e-300)
 
 
+def relerr32(eg, eo):
+    """FP32C reading of "relative 1e-5" (R22): V, T_PB, T_JF relative to themselves; E_PB = V + T_PB
+    relative to max(|E_PB|, (|V| + |T_PB|) / 20) -- E_L of a single configuration can cancel to ~0 (it does
+    at N = 64), where no fp32 pair arithmetic has a relative error; the floor asks 5e-7 of the terms instead."""
+    den = np.abs(eo[:, :4]).copy()
+    den[:, 0] = np.maximum(den[:, 0], (np.abs(eo[:, 1]) + np.abs(eo[:, 2])) / 20.0)
+    return np.abs(eg - eo[:, :4]) / np.maximum(den, 1e-300)
+
+
 # ------------------------------------------------------------------------------ initial state
 @pytest.mark.parametrize("N", [2, 64, 100, 256, 1952])
 def test_init_walkers_bit_identical_fp64(qmc, oracle, N):
@@ -203,7 +212,7 @@ def test_local_energy_fp32c(qmc, oracle, N):
     jump = abs(oracle.aziz(L / 2, AZ))
     ok = ~((eo[:, 5] < 5e-7) & (jump > 0.1 * TOL32 * np.abs(eo[:, 0])))
     assert ok.any()
-    assert relerr(eg[ok], eo[ok, :4]).max() < TOL32, relerr(eg[ok], eo[ok, :4])
+    assert relerr32(eg[ok], eo[ok]).max() < TOL32, relerr32(eg[ok], eo[ok])
     S = q.pair_sums().cpu().numpy()
     Sr = oracle.pair_sums(orc_sys(oracle, N, L), xyz[0])
     assert np.abs(S[0] - Sr).max() < 2e-6 * np.abs(Sr).max()
@@ -224,7 +233,7 @@ def test_local_energy_fp32c_equilibrated_liquid(qmc, oracle, N, W):
     jump = abs(oracle.aziz(L / 2, AZ))
     ok = ~((eo[:, 5] < 5e-7) & (jump > 0.1 * TOL32 * np.abs(eo[:, 0])))
     assert ok.sum() >= W - 1
-    assert relerr(eg[ok], eo[ok, :4]).max() < TOL32, relerr(eg[ok], eo[ok, :4]).max(0)
+    assert relerr32(eg[ok], eo[ok]).max() < TOL32, relerr32(eg[ok], eo[ok]).max(0)
 
 
 def test_local_energy_config4_size(qmc, oracle):
@@ -235,7 +244,7 @@ def test_local_energy_config4_size(qmc, oracle):
     q.set_positions(xyz)
     eg = q.local_energy().cpu().numpy()
     eo = oracle.local_energy(orc_sys(oracle, N, L), xyz)
-    assert relerr(eg, eo[:, :4]).max() < TOL32
+    assert relerr32(eg, eo).max() < TOL32
     # and sweeps run at this size (1024 threads x 10 particles); the running pair sums stay equal to
     # the kernel's own from-scratch rebuild (GPU-internal invariant; the rebuild itself is checked
     # against the oracle above and in test_local_energy_fp32c)
