@@ -115,7 +115,8 @@ __global__ void get_pair_sums_kernel(StateView sv, double *__restrict__ S)
 {
     const int w = blockIdx.y;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < sv.N) S[(size_t)w * sv.N + i] = sv.S[(size_t)w * sv.ld + i];
+    // the state holds raw sums of t = y^5 + z^5 - sh; u = c1 t (qmc_sweep_impl.cuh)
+    if (i < sv.N) S[(size_t)w * sv.N + i] = sv.groups[sv.group_of[w]].c1 * sv.S[(size_t)w * sv.ld + i];
 }
 
 __global__ void acceptance_kernel(StateView sv, double attempted, double *__restrict__ out)
@@ -279,6 +280,7 @@ extern "C" int qmc_create(const qmc_params *p, void *cuda_stream, void *d_state,
         G.c1 = -0.5 * G.b5;
         const double h = G.h;
         G.c0 = G.b5 / (h * h * h * h * h);
+        G.sh = 2.0 / (h * h * h * h * h);
         G.step = 0.0;
         long long k = 1;
         while (4 * k * k * k < p->N) ++k;

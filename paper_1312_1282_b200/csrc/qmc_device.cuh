@@ -26,7 +26,8 @@ struct AzizDev {            // HFD-B(HE), l.131, R3; inv_rm, rm2, Drm in coordin
 
 struct GroupDev {
     double L, h, h2;        // box edge, cutoff L/2, cutoff squared            [coordinate units]
-    double c1, c0;          // u = c1*(y^5+z^5) + c0                             [coordinate units]
+    double c1, c0;          // u = c1*(y^5+z^5) + c0 = c1*t,  t = y^5 + z^5 - sh  [coordinate units]
+    double sh;              // 2/h^5: t(h) = 0 (exactly 64 in FP32C box units)
     double b5;              // b^5 (for u', u'')                                 [coordinate units]
     double unit, inv_unit;  // Angstrom per coordinate unit and its inverse (1 in FP64, L and 1/L in FP32C)
     double origin;          // stored coordinate of x = 0 (0 in FP64, 1 in FP32C)

@@ -129,6 +129,7 @@ energy_kernel(StateView sv, double Dk, double *__restrict__ out)
     P.load(g);
     EnergyConst<Real> E;
     E.load(g, g.az);
+    const Real sh = (Real)g.sh;
 
     const Real *gpos = reinterpret_cast<const Real *>(sv.pos) + (size_t)w * 3 * ld;
     {
@@ -161,9 +162,8 @@ energy_kernel(StateView sv, double Dk, double *__restrict__ out)
                 const Real zz = rcp_pos(P.L - r);
                 const Real y2 = yy * yy, z2 = zz * zz;
                 const Real y4 = y2 * y2, z4 = z2 * z2;
-                const Real y5 = y4 * yy, z5 = z4 * zz;
-                const Real u = fma(P.c1, y5 + z5, P.c0);
-                ps += in ? u : (Real)0;
+                const Real t = fma(z4, zz, fma(y4, yy, -sh));      // raw pair sum term, u = c1 t
+                ps += in ? t : (Real)0;
                 if (kEnergy) {
                     const Real y6 = y4 * y2, z6 = z4 * z2;
                     const Real y7 = y6 * yy, z7 = z6 * zz;

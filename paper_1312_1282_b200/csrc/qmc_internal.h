@@ -28,7 +28,7 @@ struct TraceView {
     long long capacity, offset;   // offset = moves already recorded per walker
 };
 
-struct SweepPlan  { int threads, J, V, smem_bytes, ctas_per_sm; };
+struct SweepPlan  { int threads, J, V, smem_bytes, ctas_per_sm; const void *shape; };
 struct EnergyPlan { int threads, smem_bytes, ctas_per_sm; };
 
 }  // namespace qmc

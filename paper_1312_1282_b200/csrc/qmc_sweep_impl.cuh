@@ -1,0 +1,403 @@
+// qmc_sweep_impl.cuh -- the Metropolis sweep kernel.
+//
+// One CTA per walker ("each thread block serves one walker").  The walker's
+// coordinates (SoA) and running pair sums stay in shared memory for the whole call (l.175, l.323
+// "shared memory persistence"); global memory is touched once on entry and once on exit.
+//
+// Pair sums are kept in RAW units: t(r) = y^5 + z^5 - sh with y = 1/r, z = 1/(L-r), sh = 2/h^5, so that
+// u(r) = c1 t(r) (Eq.(8)/(9), R1) and t(h) = 0; S_i = sum_{j != i} t(r_ij); Delta = c1 (sum_j t_new - S_s).
+//
+// Per move (particle s, sweep t):
+//   a2  variates from Philox4x32-10(counter (s,t,walker,0), key seed), prepared 32 moves at a time
+//       by warp 0 (one move per lane, including log(xi)) into a double-buffered shared array;
+//   a3  thread tid evaluates t(|r'_s - r_j|) for its own particles (J of them, in packs of V consecutive
+//       ones read as one shared-memory vector) and keeps the values in registers;
+//   a4  the old sum is the running S_s (only the thread that owns s reads it);
+//   a5  xor-butterfly warp sums, one shared-memory exchange, then every thread adds the warp totals in
+//       the same fixed order: every thread ends with the same bits;
+//   a6  every thread takes the same decision 2*Delta > log(xi): ONE __syncthreads per move;
+//   a7  on accept each thread re-evaluates the OLD terms of its own particles and updates its own
+//       S_j += t_new - t_old; the owner of s commits the position and S_s.
+// Ownership is static, so S and the pair loops need no synchronisation.  The pair loops carry no index
+// test: the owner of s "poisons" the stored x of particle s for the duration of the move (half a box away
+// from the point the distances are taken from in FP32C, NaN in FP64) so that the self term is exactly 0;
+// r_s itself was read by every thread BEFORE the previous move's barrier (prefetch).
+//
+// FP32C (R20): a coordinate is the 23-bit grid index k of s = 1 + x/L in [1,2), held in shared memory as the
+// 32-bit fixed-point number k << 9.  a - b in wrapping 32-bit integer arithmetic IS the minimum image
+// (l.325), exactly; one I2FP gives it as fp32.  Everything after that is fp32 in box units.
+#pragma once
+#include "qmc_internal.h"
+
+namespace qmc {
+
+constexpr int kChunk = 32;                       // moves prepared at a time (one per lane of warp 0)
+
+template <typename Real> struct ModeT;
+template <> struct ModeT<double> { using Coord = double;  using Disp = double; };
+template <> struct ModeT<float>  { using Coord = int32_t; using Disp = int32_t; };
+
+// Displacement (coordinate units, already times step) and log(xi) of one move.
+template <typename Real> struct MoveRand { double logxi; typename ModeT<Real>::Disp dx, dy, dz; };
+
+// V consecutive values as one shared-memory vector access.
+template <typename E, int V> struct alignas(sizeof(E) * V) Pack { E v[V]; };
+
+// ---- FP32C coordinate codec: fp32 s in [1,2)  <->  fixed point (mantissa << 9) -------------------
+__device__ __forceinline__ int32_t enc_coord(float s) { return (int32_t)((__float_as_uint(s) & 0x7FFFFFu) << 9); }
+__device__ __forceinline__ float dec_coord(int32_t k) { return __uint_as_float(0x3F800000u | ((uint32_t)k >> 9)); }
+__device__ __forceinline__ int32_t wsub(int32_t a, int32_t b) { return (int32_t)((uint32_t)a - (uint32_t)b); }
+__device__ __forceinline__ int32_t wadd(int32_t a, int32_t b) { return (int32_t)((uint32_t)a + (uint32_t)b); }
+
+// ---- per-mode constants of the pair function -----------------------------------------------------
+template <typename Real> struct SweepConst;
+template <> struct SweepConst<double> {
+    double L, h, h2, sh;
+    __device__ __forceinline__ void load(const GroupDev &g) { L = g.L; h = g.h; h2 = g.h2; sh = g.sh; }
+};
+template <> struct SweepConst<float> {
+    __device__ __forceinline__ void load(const GroupDev &) {}      // box units: L = 1, h = 1/2, sh = 64
+};
+
+// t(r) between the point (px,py,pz) and the stored particle (X,Y,Z).
+// FP64: fold m = h - |h - |a-b|| per component (exact minimum image for |a-b| <= L), select on r^2 < h^2
+// (R2; NaN -- poison or padding -- selects 0).
+__device__ __forceinline__ double pair_t(double px, double py, double pz, double X, double Y, double Z,
+                                         double /*bias*/, const SweepConst<double> &P)
+{
+    const double mx = P.h - fabs(P.h - fabs(px - X));
+    const double my = P.h - fabs(P.h - fabs(py - Y));
+    const double mz = P.h - fabs(P.h - fabs(pz - Z));
+    const double r2 = fma(mz, mz, fma(my, my, mx * mx));
+    const double y = rsqrt_pos(r2);
+    const double r = r2 * y;
+    const double z = rcp_pos(P.L - r);
+    const double y2 = y * y, z2 = z * z;
+    const double y4 = y2 * y2, z4 = z2 * z2;
+    const double t = fma(z4, z, fma(y4, y, -P.sh));
+    return r2 < P.h2 ? t : 0.0;
+}
+// FP32C: wrapping integer difference = minimum image * 2^32; r^2 is clamped to h^2 = 1/4, where
+// y = z = 2 and t = 16*2 + (16*2 - 64) = 0 exactly, so pairs at and beyond the cutoff add exactly 0.
+// bias = 0 for a real particle, 1 for a padding slot (clamps).
+__device__ __forceinline__ float pair_t(int32_t px, int32_t py, int32_t pz, int32_t X, int32_t Y, int32_t Z,
+                                        float bias, const SweepConst<float> &)
+{
+    const float mx = __int2float_rn(wsub(px, X));
+    const float my = __int2float_rn(wsub(py, Y));
+    const float mz = __int2float_rn(wsub(pz, Z));
+    const float r2p = fmaf(mx, mx, fmaf(my, my, mz * mz));
+    const float r2 = fminf(fmaf(r2p, 0x1p-64f, bias), 0.25f);
+    const float y = rsqrt_pos(r2);
+    const float r = r2 * y;
+    const float z = rcp_pos(1.0f - r);
+    const float y2 = y * y, z2 = z * z;
+    const float y4 = y2 * y2, z4 = z2 * z2;
+    return fmaf(z4, z, fmaf(y4, y, -64.0f));
+}
+
+template <typename Real> __device__ __forceinline__ typename ModeT<Real>::Coord poison_of(typename ModeT<Real>::Coord p);
+template <> __device__ __forceinline__ double poison_of<double>(double) { return __longlong_as_double(0x7ff8000000000000LL); }
+template <> __device__ __forceinline__ int32_t poison_of<float>(int32_t p) { return (int32_t)((uint32_t)p + 0x80000000u); }
+
+// trial coordinate.  FP64: ONE rounding (bit-identical to the oracle).  FP32C: grid index + displacement
+// rounded to the grid (a symmetric proposal on the lattice of representable positions), periodic by wrap-around.
+__device__ __forceinline__ double trial_coord(double x, double d) { return __dadd_rn(x, d); }
+__device__ __forceinline__ int32_t trial_coord(int32_t x, int32_t d) { return wadd(x, d); }
+
+__device__ __forceinline__ double commit_coord(double x, double L)      // R10
+{
+    if (x >= L) x -= L;
+    if (x < 0.0) x += L;
+    return x;
+}
+__device__ __forceinline__ int32_t commit_coord(int32_t x, double) { return x; }
+
+// position of particle j in the shared S array: the V doubles of a pack are stored as V/2 chunks of 16 bytes,
+// chunk c of group g at ((g*(V/2) + c)*T + tid)*2, so that a warp's 16-byte accesses are contiguous.
+template <int T, int V>
+__device__ __forceinline__ int s_index(int j)
+{
+    if (V == 1) return j;
+    const int gi = j / (T * V), rem = j - gi * (T * V);
+    const int tid = rem / V, e = rem - tid * V;
+    return ((gi * (V / 2) + (e >> 1)) * T + tid) * 2 + (e & 1);
+}
+
+static inline int sweep_smem_bytes(int T, int J, int mode)
+{
+    const int real = (mode == QMC_FP64) ? 8 : 4;
+    const int NP = T * J;
+    return NP * 8 + 2 * kChunk * 32 + 64 * 8 + 3 * NP * real;
+}
+
+// Resident CTAs per SM the register allocator should leave room for: what shared memory allows for
+// this (T,J), capped so that fp64 code keeps >= ~80 and fp32 code >= ~48 registers plus the J retained terms.
+template <typename Real, int T, int J>
+constexpr int sweep_min_ctas()
+{
+    const int real = (int)sizeof(Real);
+    const int smem = J * T * (8 + 3 * real) + 2 * kChunk * 32 + 64 * 8 + 1024;
+    const int by_smem = (228 * 1024) / smem;
+    const int regs = (real == 8 ? 96 + 3 * J : 64 + 2 * J);
+    const int by_regs = 65536 / (regs * T);
+    int n = by_smem < by_regs ? by_smem : by_regs;
+    return n < 1 ? 1 : (n > 32 ? 32 : n);
+}
+
+// sum of the NW warp totals in a fixed pairwise order (same bits in every thread)
+template <int NW>
+__device__ __forceinline__ double sum_parts(const double *pb)
+{
+    double v[NW];
+    if (NW >= 2) {
+#pragma unroll
+        for (int i = 0; i < NW; i += 2) {
+            const double2 p = *reinterpret_cast<const double2 *>(pb + i);
+            v[i] = p.x; v[i + 1] = p.y;
+        }
+    } else {
+        v[0] = pb[0];
+    }
+#pragma unroll
+    for (int st = 1; st < NW; st *= 2)
+#pragma unroll
+        for (int i = 0; i + st < NW; i += 2 * st) v[i] += v[i + st];
+    return v[0];
+}
+
+// T threads per CTA; each thread owns J particles in G = J/V packs of V consecutive ones:
+// particle j = (g*T + tid)*V + e, g < G, e < V.  Shared arrays are padded to NP = T*J entries.
+template <typename Real, int T, int J, int V>
+__global__ void __launch_bounds__(T, (sweep_min_ctas<Real, T, J>()))
+sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
+{
+    static_assert(J % V == 0, "J must be a multiple of the vector width");
+    static_assert(V == 1 || V == 2 || V == 4, "vector width");
+    using Coord = typename ModeT<Real>::Coord;
+    using PackC = Pack<Coord, V>;
+    constexpr bool kF32 = (sizeof(Real) == 4);
+    constexpr int NP = T * J, G = J / V, nwarps = T >> 5;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = sv.N, ld = sv.ld;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int w = blockIdx.x;
+
+    double         *S    = reinterpret_cast<double *>(smem_raw);                              // [NP], permuted (s_index)
+    unsigned char  *rnd  = smem_raw + NP * 8;                                                 // [2][kChunk] 32-byte slots
+    double         *part = reinterpret_cast<double *>(smem_raw + NP * 8 + 2 * kChunk * 32);   // [2][32]
+    Coord          *x    = reinterpret_cast<Coord *>(part + 64);                              // [3][NP]
+    Coord *y = x + NP, *z = x + 2 * NP;
+    static_assert(sizeof(MoveRand<Real>) <= 32, "variate record must fit its 32-byte slot");
+
+    const GroupDev g = sv.groups[sv.group_of[w]];
+    SweepConst<Real> P;
+    P.load(g);
+    const double c2 = 2.0 * g.c1;                          // 2 Delta = c2 * (sum t_new - S_s)
+    // proposal half-width: FP64 exactly the caller's step [A]; FP32C in grid units (2^-23 box)
+    const double step = kF32 ? g.step * g.inv_unit * 8388608.0 : g.step;
+    const uint32_t wid = sv.walker_id_base + (uint32_t)w;
+
+    // a1: walker state global -> shared, once per call
+    Real *gpos = reinterpret_cast<Real *>(sv.pos) + (size_t)w * 3 * ld;
+    double *gS = sv.S + (size_t)w * ld;
+    for (int j = tid; j < NP; j += T) {
+        Coord cx, cy, cz;
+        double s = 0.0;
+        if (j < N) {
+            if constexpr (kF32) { cx = enc_coord(gpos[j]); cy = enc_coord(gpos[ld + j]); cz = enc_coord(gpos[2 * ld + j]); }
+            else                { cx = gpos[j]; cy = gpos[ld + j]; cz = gpos[2 * ld + j]; }
+            s = gS[j];
+        } else {                                            // padding: NaN selects 0 in FP64; FP32C uses the bias
+            if constexpr (kF32) { cx = 0; cy = 0; cz = 0; }
+            else                { cx = cy = cz = poison_of<Real>(Coord(0)); }
+        }
+        x[j] = cx; y[j] = cy; z[j] = cz;
+        S[s_index<T, V>(j)] = s;
+    }
+
+    // per-pack clamp bias of this thread (FP32C): 1 for padding packs.  Requires N % V == 0 (planner).
+    float bias[G];
+#pragma unroll
+    for (int gi = 0; gi < G; ++gi) bias[gi] = ((gi * T + tid) * V < N) ? 0.0f : 1.0f;
+
+    const uint32_t total = (uint32_t)n_sweeps * (uint32_t)N;
+
+    // a2: variates of moves [chunk*32, chunk*32+32) -> rnd[buf]
+    auto produce = [&](uint32_t chunk, int buf) {
+        if (warp != 0) return;
+        const uint32_t m = chunk * kChunk + lane;
+        if (m >= total) return;
+        const uint32_t q = m / (uint32_t)N;
+        const uint32_t s = m - q * (uint32_t)N;
+        const uint4 r = philox4x32_10(make_uint4(s, t0 + q, wid, 0u), key);
+        MoveRand<Real> mr;
+        const double ax = __dmul_rn(step, word_to_pm1(r.x));
+        const double ay = __dmul_rn(step, word_to_pm1(r.y));
+        const double az = __dmul_rn(step, word_to_pm1(r.z));
+        if constexpr (kF32) {
+            mr.dx = (int32_t)((uint32_t)__double2int_rn(ax) << 9);
+            mr.dy = (int32_t)((uint32_t)__double2int_rn(ay) << 9);
+            mr.dz = (int32_t)((uint32_t)__double2int_rn(az) << 9);
+        } else {
+            mr.dx = ax; mr.dy = ay; mr.dz = az;
+        }
+        mr.logxi = log(word_to_unit(r.w));
+        *reinterpret_cast<MoveRand<Real> *>(rnd + (buf * kChunk + lane) * 32) = mr;
+    };
+    auto fetch = [&](uint32_t m) {
+        return *reinterpret_cast<const MoveRand<Real> *>(rnd + ((int)((m >> 5) & 1) * kChunk + (int)(m & (kChunk - 1))) * 32);
+    };
+    produce(0, 0);
+    __syncthreads();
+
+    unsigned long long n_acc = 0;
+    int s = 0;
+    MoveRand<Real> mr = fetch(0);
+    Coord xs = x[0], ys = y[0], zs = z[0];                 // the moved particle (prefetched one move ahead)
+    __syncthreads();                                       // ... before its owner poisons it
+    for (uint32_t m = 0; m < total; ++m) {
+        if ((m & (kChunk - 1)) == 0) produce((m >> 5) + 1, (int)(((m >> 5) + 1) & 1));   // published by this move's barrier
+        const Coord tx = trial_coord(xs, mr.dx);
+        const Coord ty = trial_coord(ys, mr.dy);
+        const Coord tz = trial_coord(zs, mr.dz);
+        const double logxi = mr.logxi;
+        const bool owner = (tid == (s / V) % T);
+        if (owner) x[s] = poison_of<Real>(tx);             // self term = 0 (nobody else reads x[s] during this move)
+
+        // prefetch the next move: its particle cannot change in this move (N >= 3; else re-read below)
+        const int sn = (s + 1 == N) ? 0 : s + 1;
+        const Coord xn = x[sn], yn = y[sn], zn = z[sn];
+        if (m + 1 < total) mr = fetch(m + 1);
+
+        // a3: trial terms of this thread's particles
+        Real un[J];
+        Real accr = (Real)0;
+#pragma unroll
+        for (int gi = 0; gi < G; ++gi) {
+            const int base = (gi * T + tid) * V;
+            const PackC X = *reinterpret_cast<const PackC *>(x + base);
+            const PackC Y = *reinterpret_cast<const PackC *>(y + base);
+            const PackC Z = *reinterpret_cast<const PackC *>(z + base);
+#pragma unroll
+            for (int e = 0; e < V; ++e) {
+                un[gi * V + e] = pair_t(tx, ty, tz, X.v[e], Y.v[e], Z.v[e], bias[gi], P);
+                accr += un[gi * V + e];
+            }
+        }
+        double acc = (double)accr;
+        if (owner) acc -= S[s_index<T, V>(s)];             // a4: sum_j t_new - S_s
+
+        // a5: block sum, identical bits in every thread
+        double tot = warp_sum(acc);
+        if (nwarps > 1) {
+            double *pb = part + (int)(m & 1) * 32;
+            if (lane == 0) pb[warp] = tot;
+            __syncthreads();
+            tot = sum_parts<nwarps>(pb);
+        } else {
+            __syncwarp();
+        }
+
+        // a6: decision (Eq.(5), strict, log form: R8)
+        const double margin = fma(c2, tot, -logxi);
+        const bool accept = margin > 0.0;
+        if (tr.dec != nullptr) {
+            if (tid == 0 && w >= tr.w_begin && w < tr.w_end) {
+                const long long k = tr.offset + m;
+                if (k < tr.capacity) {
+                    const long long idx = (long long)(w - tr.w_begin) * tr.capacity + k;
+                    tr.dec[idx] = accept ? 1 : 0;
+                    if (tr.margin != nullptr) tr.margin[idx] = margin;
+                }
+            }
+        }
+
+        // a7: commit and update the running pair sums
+        if (accept) {
+            if (kF32 && owner) x[s] = poison_of<Real>(xs);  // distances are now taken from the old position
+#pragma unroll
+            for (int gi = 0; gi < G; ++gi) {
+                const int base = (gi * T + tid) * V;
+                const PackC X = *reinterpret_cast<const PackC *>(x + base);
+                const PackC Y = *reinterpret_cast<const PackC *>(y + base);
+                const PackC Z = *reinterpret_cast<const PackC *>(z + base);
+                if constexpr (V == 1) {
+                    const Real to = pair_t(xs, ys, zs, X.v[0], Y.v[0], Z.v[0], bias[gi], P);
+                    S[base] += (double)(un[gi] - to);
+                } else {
+#pragma unroll
+                    for (int c = 0; c < V / 2; ++c) {
+                        double2 *sp = reinterpret_cast<double2 *>(S + ((gi * (V / 2) + c) * T + tid) * 2);
+                        double2 sv2 = *sp;
+                        const Real t0o = pair_t(xs, ys, zs, X.v[2 * c], Y.v[2 * c], Z.v[2 * c], bias[gi], P);
+                        const Real t1o = pair_t(xs, ys, zs, X.v[2 * c + 1], Y.v[2 * c + 1], Z.v[2 * c + 1], bias[gi], P);
+                        sv2.x += (double)(un[gi * V + 2 * c] - t0o);
+                        sv2.y += (double)(un[gi * V + 2 * c + 1] - t1o);
+                        *sp = sv2;
+                    }
+                }
+            }
+            if (owner) {
+                S[s_index<T, V>(s)] += tot;
+                x[s] = commit_coord(tx, g.L);
+                y[s] = commit_coord(ty, g.L);
+                z[s] = commit_coord(tz, g.L);
+            }
+            ++n_acc;
+        } else if (owner) {
+            x[s] = xs;                                      // undo the poison
+        }
+        s = sn;
+        xs = xn; ys = yn; zs = zn;
+        if (N < 3) {                                        // degenerate: the next particle may just have moved
+            __syncthreads();
+            xs = x[s]; ys = y[s]; zs = z[s];
+            __syncthreads();
+        }
+    }
+    __syncthreads();
+
+    // a8: shared -> global, once per call
+    for (int j = tid; j < N; j += T) {
+        if constexpr (kF32) { gpos[j] = dec_coord(x[j]); gpos[ld + j] = dec_coord(y[j]); gpos[2 * ld + j] = dec_coord(z[j]); }
+        else                { gpos[j] = x[j]; gpos[ld + j] = y[j]; gpos[2 * ld + j] = z[j]; }
+        gS[j] = S[s_index<T, V>(j)];
+    }
+    if (tid == 0) sv.n_acc[w] += n_acc;
+}
+
+// ---- host side: one table entry per compiled (T, J, V) shape ----------------------------------------
+struct SweepShape {
+    int T, J, V;
+    cudaError_t (*launch)(qmc_ctx *c, int n_sweeps, int smem);
+    int (*occupancy)(int smem);
+};
+
+template <typename Real, int T, int J, int V>
+static cudaError_t shape_launch(qmc_ctx *c, int n_sweeps, int smem)
+{
+    const uint2 key = make_uint2((uint32_t)(c->seed & 0xFFFFFFFFull), (uint32_t)(c->seed >> 32));
+    auto kern = sweep_kernel<Real, T, J, V>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<c->W, T, smem, c->stream>>>(c->sv, c->trace, key, c->t, n_sweeps);
+    return cudaGetLastError();
+}
+
+template <typename Real, int T, int J, int V>
+static int shape_occupancy(int smem)
+{
+    int n = 0;
+    auto kern = sweep_kernel<Real, T, J, V>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, T, smem) != cudaSuccess) return 0;
+    return n;
+}
+
+#define QMC_SHAPE_ENTRY(Real, TT, JJ, VV) {TT, JJ, VV, shape_launch<Real, TT, JJ, VV>, shape_occupancy<Real, TT, JJ, VV>},
+
+const SweepShape *sweep_shapes_f32(int *n);
+const SweepShape *sweep_shapes_f64(int *n);
+
+}  // namespace qmc
