@@ -96,6 +96,43 @@ __device__ __forceinline__ float pair_t(int32_t px, int32_t py, int32_t pz, int3
     return fmaf(z4, z, fmaf(y4, y, -64.0f));
 }
 
+// ---- packed fp32 (Blackwell FFMA2 / FMUL2 / FADD2: two fp32 lanes per 64-bit register pair, one issue slot) ----
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void upk2(f32x2 r, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(r)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+
+// Two FP32C pair terms at once: same arithmetic as pair_t(int...) but r^2 stays scaled by 2^64 up to the
+// reciprocal square root (y' = y 2^-32, q = r 2^32), which saves the scaling multiply; the clamp is at
+// 2^62 = h^2 2^64 and bias2 holds 0 or 2^63 per lane (padding).  Every power of two is exact, so the
+// results are bit-identical to the scalar form.
+__device__ __forceinline__ f32x2 pair_t2(int32_t px, int32_t py, int32_t pz, int32_t X0, int32_t X1, int32_t Y0, int32_t Y1,
+                                         int32_t Z0, int32_t Z1, f32x2 bias2)
+{
+    const f32x2 mx = pk2(__int2float_rn(wsub(px, X0)), __int2float_rn(wsub(px, X1)));
+    const f32x2 my = pk2(__int2float_rn(wsub(py, Y0)), __int2float_rn(wsub(py, Y1)));
+    const f32x2 mz = pk2(__int2float_rn(wsub(pz, Z0)), __int2float_rn(wsub(pz, Z1)));
+    const f32x2 r2p = fma2(mx, mx, fma2(my, my, fma2(mz, mz, bias2)));
+    float a, b;
+    upk2(r2p, a, b);
+    a = fminf(a, 0x1p62f);
+    b = fminf(b, 0x1p62f);
+    const float ya = rsqrt_pos(a), yb = rsqrt_pos(b);                   // y 2^-32
+    const f32x2 r2c = pk2(a, b), yp = pk2(ya, yb);
+    const f32x2 q = mul2(r2c, yp);                                      // r 2^32
+    const f32x2 omr = fma2(q, pk2(-0x1p-32f, -0x1p-32f), pk2(1.0f, 1.0f));
+    float oa, ob;
+    upk2(omr, oa, ob);
+    const f32x2 z = pk2(rcp_pos(oa), rcp_pos(ob));
+    const f32x2 y = mul2(yp, pk2(0x1p32f, 0x1p32f));
+    const f32x2 y2 = mul2(y, y), z2 = mul2(z, z);
+    const f32x2 y4 = mul2(y2, y2), z4 = mul2(z2, z2);
+    return fma2(z4, z, fma2(y4, y, pk2(-64.0f, -64.0f)));
+}
+
 template <typename Real> __device__ __forceinline__ typename ModeT<Real>::Coord poison_of(typename ModeT<Real>::Coord p);
 template <> __device__ __forceinline__ double poison_of<double>(double) { return __longlong_as_double(0x7ff8000000000000LL); }
 template <> __device__ __forceinline__ int32_t poison_of<float>(int32_t p) { return (int32_t)((uint32_t)p + 0x80000000u); }
@@ -139,7 +176,7 @@ constexpr int sweep_min_ctas()
     const int real = (int)sizeof(Real);
     const int smem = J * T * (8 + 3 * real) + 2 * kChunk * 32 + 64 * 8 + 1024;
     const int by_smem = (228 * 1024) / smem;
-    const int regs = (real == 8 ? 96 + 3 * J : 64 + 2 * J);
+    const int regs = (real == 8 ? 96 + 3 * J : 40 + 3 * J);
     const int by_regs = 65536 / (regs * T);
     int n = by_smem < by_regs ? by_smem : by_regs;
     return n < 1 ? 1 : (n > 32 ? 32 : n);
@@ -177,6 +214,7 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
     using Coord = typename ModeT<Real>::Coord;
     using PackC = Pack<Coord, V>;
     constexpr bool kF32 = (sizeof(Real) == 4);
+    constexpr bool kPacked = kF32 && V >= 2;              // two pair terms per FFMA2-class instruction
     constexpr int NP = T * J, G = J / V, nwarps = T >> 5;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = sv.N, ld = sv.ld;
@@ -220,6 +258,9 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
     float bias[G];
 #pragma unroll
     for (int gi = 0; gi < G; ++gi) bias[gi] = ((gi * T + tid) * V < N) ? 0.0f : 1.0f;
+    f32x2 bias2[G];
+#pragma unroll
+    for (int gi = 0; gi < G; ++gi) bias2[gi] = ((gi * T + tid) * V < N) ? pk2(0.0f, 0.0f) : pk2(0x1p63f, 0x1p63f);
 
     const uint32_t total = (uint32_t)n_sweeps * (uint32_t)N;
 
@@ -271,18 +312,39 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
         if (m + 1 < total) mr = fetch(m + 1);
 
         // a3: trial terms of this thread's particles
-        Real un[J];
+        Real un[kPacked ? 1 : J];
+        f32x2 un2[kPacked ? J / 2 : 1];
         Real accr = (Real)0;
+        if constexpr (kPacked) {
+            f32x2 acc2 = pk2(0.0f, 0.0f);
 #pragma unroll
-        for (int gi = 0; gi < G; ++gi) {
-            const int base = (gi * T + tid) * V;
-            const PackC X = *reinterpret_cast<const PackC *>(x + base);
-            const PackC Y = *reinterpret_cast<const PackC *>(y + base);
-            const PackC Z = *reinterpret_cast<const PackC *>(z + base);
+            for (int gi = 0; gi < G; ++gi) {
+                const int base = (gi * T + tid) * V;
+                const PackC X = *reinterpret_cast<const PackC *>(x + base);
+                const PackC Y = *reinterpret_cast<const PackC *>(y + base);
+                const PackC Z = *reinterpret_cast<const PackC *>(z + base);
 #pragma unroll
-            for (int e = 0; e < V; ++e) {
-                un[gi * V + e] = pair_t(tx, ty, tz, X.v[e], Y.v[e], Z.v[e], bias[gi], P);
-                accr += un[gi * V + e];
+                for (int e = 0; e < V; e += 2) {
+                    const f32x2 t2 = pair_t2(tx, ty, tz, X.v[e], X.v[e + 1], Y.v[e], Y.v[e + 1], Z.v[e], Z.v[e + 1], bias2[gi]);
+                    un2[(gi * V + e) / 2] = t2;
+                    acc2 = add2(acc2, t2);
+                }
+            }
+            float a0, a1;
+            upk2(acc2, a0, a1);
+            accr = a0 + a1;
+        } else {
+#pragma unroll
+            for (int gi = 0; gi < G; ++gi) {
+                const int base = (gi * T + tid) * V;
+                const PackC X = *reinterpret_cast<const PackC *>(x + base);
+                const PackC Y = *reinterpret_cast<const PackC *>(y + base);
+                const PackC Z = *reinterpret_cast<const PackC *>(z + base);
+#pragma unroll
+                for (int e = 0; e < V; ++e) {
+                    un[gi * V + e] = pair_t(tx, ty, tz, X.v[e], Y.v[e], Z.v[e], bias[gi], P);
+                    accr += un[gi * V + e];
+                }
             }
         }
         double acc = (double)accr;
@@ -330,10 +392,19 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
                     for (int c = 0; c < V / 2; ++c) {
                         double2 *sp = reinterpret_cast<double2 *>(S + ((gi * (V / 2) + c) * T + tid) * 2);
                         double2 sv2 = *sp;
-                        const Real t0o = pair_t(xs, ys, zs, X.v[2 * c], Y.v[2 * c], Z.v[2 * c], bias[gi], P);
-                        const Real t1o = pair_t(xs, ys, zs, X.v[2 * c + 1], Y.v[2 * c + 1], Z.v[2 * c + 1], bias[gi], P);
-                        sv2.x += (double)(un[gi * V + 2 * c] - t0o);
-                        sv2.y += (double)(un[gi * V + 2 * c + 1] - t1o);
+                        if constexpr (kPacked) {
+                            const f32x2 to2 = pair_t2(xs, ys, zs, X.v[2 * c], X.v[2 * c + 1], Y.v[2 * c], Y.v[2 * c + 1],
+                                                      Z.v[2 * c], Z.v[2 * c + 1], bias2[gi]);
+                            float d0, d1;
+                            upk2(sub2(un2[(gi * V) / 2 + c], to2), d0, d1);
+                            sv2.x += (double)d0;
+                            sv2.y += (double)d1;
+                        } else {
+                            const Real t0o = pair_t(xs, ys, zs, X.v[2 * c], Y.v[2 * c], Z.v[2 * c], bias[gi], P);
+                            const Real t1o = pair_t(xs, ys, zs, X.v[2 * c + 1], Y.v[2 * c + 1], Z.v[2 * c + 1], bias[gi], P);
+                            sv2.x += (double)(un[gi * V + 2 * c] - t0o);
+                            sv2.y += (double)(un[gi * V + 2 * c + 1] - t1o);
+                        }
                         *sp = sv2;
                     }
                 }
