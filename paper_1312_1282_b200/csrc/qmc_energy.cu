@@ -242,9 +242,9 @@ static cudaError_t launch_e(qmc_ctx *c, double *d_out, bool energy)
 cudaError_t launch_energy(qmc_ctx *c, double *d_out, bool energy)
 {
     c->launches += 1;
+    if (c->p.mode != QMC_FP64) return launch_energy_f32(c, d_out, energy);     // qmc_energy_f32.cu
     const int T = c->energy_plan.threads;
-#define X(TT) if (T == TT) return c->p.mode == QMC_FP64 ? launch_e<double, TT>(c, d_out, energy) \
-                                                        : launch_e<float, TT>(c, d_out, energy);
+#define X(TT) if (T == TT) return launch_e<double, TT>(c, d_out, energy);
     QMC_ENERGY_THREADS(X)
 #undef X
     return cudaErrorInvalidValue;
@@ -252,6 +252,7 @@ cudaError_t launch_energy(qmc_ctx *c, double *d_out, bool energy)
 
 bool plan_energy(qmc_ctx *c, EnergyPlan *out)
 {
+    if (c->p.mode != QMC_FP64) return plan_energy_f32(c, out);
     const int N = c->p.N;
     int T = 32;
     while (T < N && T < 256) T *= 2;
@@ -263,13 +264,9 @@ bool plan_energy(qmc_ctx *c, EnergyPlan *out)
     out->smem_bytes = energy_smem_bytes(c->ld, c->p.mode);
     if (out->smem_bytes > 227 * 1024) return false;
     int occ = 0;
-#define X(TT) if (T == TT) { \
-        if (c->p.mode == QMC_FP64) { auto k = energy_kernel<double, TT, true>; \
+#define X(TT) if (T == TT) { auto k = energy_kernel<double, TT, true>; \
             cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, out->smem_bytes); \
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, TT, out->smem_bytes); } \
-        else { auto k = energy_kernel<float, TT, true>; \
-            cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, out->smem_bytes); \
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, TT, out->smem_bytes); } }
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, TT, out->smem_bytes); }
     QMC_ENERGY_THREADS(X)
 #undef X
     out->ctas_per_sm = occ;

@@ -1,0 +1,360 @@
+// qmc_energy_f32.cu -- FP32C local-energy estimator over all pairs and the
+// from-scratch rebuild of the running pair sums S_i (R17).
+//
+// One CTA per walker; coordinates in shared memory as 32-bit fixed point (qmc_f32c.cuh), so the signed
+// minimum image of a pair is ONE wrapping integer subtraction.  The particles are cut into blocks of 32.
+// A warp owns an i-block (lane = particle i; grad_i log psi, lap_i log psi, S_i and V stay in registers --
+// the scatter-free layout of PAPER.md l.527's "extra memory to store wavefunction derivatives") and
+// streams the j-blocks from shared memory (every lane reads the same j: broadcast).  Two j per
+// instruction: all pair arithmetic is packed f32x2.
+//
+//   G_i      = sum_{j != i} u'(r_ij) d_ij / r_ij,     u'/r = 5/2 b^5 y (y^6 - z^6)
+//   Lambda_i = sum_{j != i} [u'' + 2 u'/r]                 = -b^5 (10 y^7 + z^6 (15 z + 5 y))
+//   V        = sum_{i<j, r<h} V_Aziz(r_ij)                 (HFD-B(HE), truncated at h, R3)
+//   T_PB = -Dk sum_i (Lambda_i + |G_i|^2),  T_JF = -Dk/2 sum_i Lambda_i,  E_PB = V + T_PB      (R14)
+// with y = 1/r, z = 1/(L-r), box units (L = 1, h = 1/2).
+//
+// No per-pair cutoff test.  r^2 is CLAMPED to h^2, where y = z = 2 exactly, so a pair at or beyond the
+// cutoff contributes exactly 0 to S_i and G_i, and exactly the constants K_L = 3840 (lap term) and
+// K_V = V(h) to the other two sums; the kernel counts the pairs inside the cutoff (one integer compare) and
+// removes (pairs - inside) K afterwards in fp64.  Only the j-block that contains the warp's own particles
+// (self pair, V for j > i only) and a ragged last block take a slower tile with explicit selects.
+// V is evaluated only in tiles with j-block > i-block (+ the diagonal tile), i.e. once per unordered pair.
+//
+// R20: per-pair terms are fp32; 16 consecutive j are summed in fp32 (two packed lanes of 8) and then added
+// to fp64 accumulators.
+#include "qmc_internal.h"
+#include "qmc_f32c.cuh"
+
+namespace qmc {
+
+namespace {
+
+constexpr float kClamp = 0x1p62f;              // h^2 2^64
+constexpr int   kClampBits = 0x5E800000;       // bit pattern of 2^62
+
+// HFD-B(HE) constants for packed fp32 evaluation.  Every constant that multiplies into the steep
+// repulsive exponential or the dispersion sum is folded (in fp64, on load) into ONE rounded coefficient
+// or carried as hi + lo, so that no fp32 rounding of a CONSTANT puts a systematic relative error on
+// every pair (the box-unit value of r_m is an arbitrary real number):
+//   rep  = eps A 2^(a1 r + a2 r^2),  a1 = -alpha log2(e) / r_m,  a2 = beta log2(e) / r_m^2   (hi + lo)
+//   disp = w^3 (k6 + w (k8 + w k10)),  w = fl(r_m^2) y^2,  k_n = eps c_n (r_m^2 / fl(r_m^2))^(n/2)
+//   F    = 2^(-log2(e) max(D r_m y - 1, 0)^2)                                     (D r_m hi + lo)
+struct AzizF32 {
+    f32x2 a1h, a1l, a2h, a2l, epsA, epsAln2, rm2, nk6, nk8, nk10, Drm, Drml;
+    __device__ __forceinline__ void load(const AzizDev &a)
+    {
+        const double log2e = 1.4426950408889634, ln2 = 0.6931471805599453;
+        auto split = [](double v, f32x2 &hi, f32x2 &lo) {
+            const float h = __double2float_rn(v);
+            hi = pk1(h);
+            lo = pk1(__double2float_rn(v - (double)h));
+        };
+        split(-a.alpha * a.inv_rm * log2e, a1h, a1l);
+        split(a.beta * a.inv_rm * a.inv_rm * log2e, a2h, a2l);
+        const float eA = (float)(a.eps * a.A);
+        epsA = pk1(eA);
+        epsAln2 = pk1((float)((double)eA * ln2));
+        const float rm2f = (float)a.rm2;
+        rm2 = pk1(rm2f);
+        const double q = a.rm2 / (double)rm2f;            // 1 + rounding error of fl(r_m^2)
+        nk6 = pk1((float)(-a.eps * a.c6 * q * q * q));
+        nk8 = pk1((float)(-a.eps * a.c8 * q * q * q * q));
+        nk10 = pk1((float)(-a.eps * a.c10 * q * q * q * q * q));
+        split(a.Drm, Drm, Drml);
+    }
+};
+
+// Everything the pair arithmetic of two j produces.
+struct Pair2 {
+    f32x2 mx, my, mz;      // signed minimum image, 2^32 box units
+    f32x2 r2c;             // min(r^2, h^2) 2^64
+    f32x2 yp, q;           // y 2^-32 (hardware rsqrt), r 2^32
+    f32x2 y, z;            // 1/r, 1/(1-r)
+    f32x2 y2, z2, y4, z4;
+    float a, b;            // the two lanes of r2c
+};
+
+__device__ __forceinline__ Pair2 pair_geom(int32_t xi, int32_t yi, int32_t zi, int32_t X0, int32_t X1, int32_t Y0, int32_t Y1,
+                                           int32_t Z0, int32_t Z1, f32x2 bias2, int32_t zero)
+{
+    Pair2 p;
+    p.mx = pk2(__int2float_rn(wsub3(xi, X0, zero)), __int2float_rn(wsub3(xi, X1, zero)));
+    p.my = pk2(__int2float_rn(wsub3(yi, Y0, zero)), __int2float_rn(wsub3(yi, Y1, zero)));
+    p.mz = pk2(__int2float_rn(wsub3(zi, Z0, zero)), __int2float_rn(wsub3(zi, Z1, zero)));
+    const f32x2 r2p = fma2(p.mx, p.mx, fma2(p.my, p.my, fma2(p.mz, p.mz, bias2)));
+    upk2(r2p, p.a, p.b);
+    p.a = fminf(p.a, kClamp);
+    p.b = fminf(p.b, kClamp);
+    p.r2c = pk2(p.a, p.b);
+    p.yp = pk2(rsqrt_pos(p.a), rsqrt_pos(p.b));
+    p.q = mul2(p.r2c, p.yp);
+    const f32x2 omr = fma2(p.q, pk1(-0x1p-32f), pk1(1.0f));
+    float oa, ob;
+    upk2(omr, oa, ob);
+    p.z = pk2(rcp_pos(oa), rcp_pos(ob));
+    p.y = mul2(p.yp, pk1(0x1p32f));
+    p.y2 = mul2(p.y, p.y);
+    p.z2 = mul2(p.z, p.z);
+    p.y4 = mul2(p.y2, p.y2);
+    p.z4 = mul2(p.z2, p.z2);
+    return p;
+}
+
+// t = y^5 + z^5 - 64 (raw pair-sum term, u = c1 t); exactly 0 at the clamp
+__device__ __forceinline__ f32x2 pair_t(const Pair2 &p) { return fma2(p.z4, p.z, fma2(p.y4, p.y, pk1(-64.0f))); }
+
+// HFD-B(HE) of the two pairs in K.  The hardware rsqrt is first refined by one Newton step (the seed is
+// good to ~2^-22 and the repulsive exponential amplifies a relative error of r ~11x).
+__device__ __forceinline__ f32x2 aziz2(const Pair2 &p, const AzizF32 &E)
+{
+    const f32x2 e = fma2(mul2(p.q, pk1(-1.0f)), p.yp, pk1(1.0f));          // 1 - r^2 y0^2
+    const f32x2 y = fma2(mul2(p.y, pk1(0.5f)), e, p.y);
+    const f32x2 r = mul2(mul2(p.r2c, pk1(0x1p-64f)), y);
+    const f32x2 w = mul2(E.rm2, mul2(y, y));
+    const f32x2 w3 = mul2(mul2(w, w), w);
+    const f32x2 ndisp = mul2(w3, fma2(w, fma2(w, E.nk10, E.nk8), E.nk6));   // -disp
+    const f32x2 t = fma2(E.Drml, y, fma2(E.Drm, y, pk1(-1.0f)));           // D/x - 1
+    float ta, tb;
+    upk2(t, ta, tb);
+    const f32x2 tc = pk2(fmaxf(ta, 0.0f), fmaxf(tb, 0.0f));                // F = 1 for x >= D
+    const f32x2 fa = mul2(mul2(tc, tc), pk1(-1.4426950408889634f));
+    float f0, f1;
+    upk2(fa, f0, f1);
+    const f32x2 F = pk2(ex2_approx(f0), ex2_approx(f1));
+    const f32x2 t1 = fma2(E.a2h, r, E.a1h);
+    const f32x2 ah = mul2(r, t1);
+    f32x2 al = fma2(r, t1, mul2(ah, pk1(-1.0f)));                          // exact residual of the product
+    al = fma2(r, fma2(E.a2l, r, E.a1l), al);
+    float h0, h1;
+    upk2(ah, h0, h1);
+    const f32x2 e2 = pk2(ex2_approx(h0), ex2_approx(h1));
+    const f32x2 rep = fma2(mul2(e2, E.epsAln2), al, mul2(e2, E.epsA));     // eps A 2^ah (1 + ln2 al)
+    return fma2(F, ndisp, rep);
+}
+
+struct Acc32 { f32x2 gx, gy, gz, lam, s, v; };
+struct Acc64 { double gx, gy, gz, lam, s, v; };
+
+// 16 consecutive j (4 vector loads per coordinate) against this lane's particle.
+//   kSlow: per-pair selects (self pair, j >= N, V only for j > i); kV: evaluate the potential.
+template <bool kEnergy, bool kV, bool kSlow>
+__device__ __forceinline__ void tile16(const int32_t *__restrict__ x, const int32_t *__restrict__ y, const int32_t *__restrict__ z,
+                                       int j0, int i, int N, int32_t xi, int32_t yi, int32_t zi, const AzizF32 &E,
+                                       int32_t zero, Acc64 &A, int &n_in)
+{
+    Acc32 P;
+    P.gx = P.gy = P.gz = P.lam = P.s = P.v = pk1(0.0f);
+#pragma unroll
+    for (int g = 0; g < 4; ++g) {
+        const int4 X = *reinterpret_cast<const int4 *>(x + j0 + 4 * g);
+        const int4 Y = *reinterpret_cast<const int4 *>(y + j0 + 4 * g);
+        const int4 Z = *reinterpret_cast<const int4 *>(z + j0 + 4 * g);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int ja = j0 + 4 * g + 2 * h, jb = ja + 1;
+            f32x2 bias2 = pk1(0.0f);
+            if (kSlow) bias2 = pk2((ja == i || ja >= N) ? 0x1p63f : 0.0f, (jb == i || jb >= N) ? 0x1p63f : 0.0f);
+            const Pair2 p = h == 0 ? pair_geom(xi, yi, zi, X.x, X.y, Y.x, Y.y, Z.x, Z.y, bias2, zero)
+                                   : pair_geom(xi, yi, zi, X.z, X.w, Y.z, Y.w, Z.z, Z.w, bias2, zero);
+            const bool ina = __float_as_int(p.a) < kClampBits, inb = __float_as_int(p.b) < kClampBits;
+            P.s = add2(P.s, pair_t(p));
+            if (kEnergy) {
+                const f32x2 y6 = mul2(p.y4, p.y2), z6 = mul2(p.z4, p.z2);
+                const f32x2 gm = mul2(p.y, sub2(y6, z6));                                    // (u'/r) / (5/2 b^5)
+                P.gx = fma2(gm, p.mx, P.gx);
+                P.gy = fma2(gm, p.my, P.gy);
+                P.gz = fma2(gm, p.mz, P.gz);
+                const f32x2 y7 = mul2(y6, p.y);
+                const f32x2 inner = fma2(p.z, pk1(15.0f), mul2(p.y, pk1(5.0f)));
+                f32x2 lt = fma2(y7, pk1(10.0f), mul2(z6, inner));                            // -(u'' + 2u'/r) / b^5
+                if (kSlow) {
+                    float la, lb;
+                    upk2(lt, la, lb);
+                    lt = pk2(ina ? la : 0.0f, inb ? lb : 0.0f);
+                } else {
+                    n_in += (ina ? 1 : 0) + (inb ? 1 : 0);
+                }
+                P.lam = add2(P.lam, lt);
+                if (kV) {
+                    f32x2 vp = aziz2(p, E);
+                    if (kSlow) {
+                        float va, vb;
+                        upk2(vp, va, vb);
+                        vp = pk2((ina && ja > i) ? va : 0.0f, (inb && jb > i) ? vb : 0.0f);
+                    }
+                    P.v = add2(P.v, vp);
+                }
+            }
+        }
+    }
+    A.s += (double)hsum2(P.s);
+    if (kEnergy) {
+        A.gx += (double)hsum2(P.gx);
+        A.gy += (double)hsum2(P.gy);
+        A.gz += (double)hsum2(P.gz);
+        A.lam += (double)hsum2(P.lam);
+        if (kV) A.v += (double)hsum2(P.v);
+    }
+}
+
+template <int T, bool kEnergy>
+__global__ void __launch_bounds__(T, (T <= 128 ? 4 : (T <= 256 ? 2 : 1)))
+energy32_kernel(StateView sv, double Dk, double *__restrict__ out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = sv.N, ld = sv.ld;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int nwarps = T >> 5;
+    const int w = blockIdx.x;
+    const int nblk = (N + 31) >> 5, NP = nblk << 5;
+
+    double  *red = reinterpret_cast<double *>(smem_raw);              // [3][32]
+    int32_t *x   = reinterpret_cast<int32_t *>(red + 96);             // [3][NP]
+    int32_t *y = x + NP, *z = x + 2 * NP;
+
+    const GroupDev g = sv.groups[sv.group_of[w]];
+    AzizF32 E;
+    E.load(g.az);
+
+    const float *gpos = reinterpret_cast<const float *>(sv.pos) + (size_t)w * 3 * ld;
+    for (int j = tid; j < NP; j += T) {
+        const bool in = j < N;
+        x[j] = in ? enc_coord(gpos[j]) : 0;
+        y[j] = in ? enc_coord(gpos[ld + j]) : 0;
+        z[j] = in ? enc_coord(gpos[2 * ld + j]) : 0;
+    }
+    if (tid == 0) *reinterpret_cast<int32_t *>(red + 95) = 0;
+    __syncthreads();
+    const int32_t zero = opaque_zero(reinterpret_cast<int32_t *>(red + 95));
+
+    // V of a clamped pair, by the same instructions every clamped pair goes through
+    float KV = 0.0f;
+    if (kEnergy) {
+        const Pair2 pc = pair_geom(0, 0, 0, 0, 0, 0, 0, 0, 0, pk1(0x1p63f), zero);
+        float va, vb;
+        upk2(aziz2(pc, E), va, vb);
+        KV = va;
+    }
+
+    const bool ragged = (N & 31) != 0;
+    double tLam = 0.0, tG2 = 0.0, tV = 0.0;
+    for (int A = warp; A < nblk; A += nwarps) {
+        const int i = (A << 5) + lane;
+        const bool live = i < N;
+        const int ic = live ? i : N - 1;
+        const int32_t xi = x[ic], yi = y[ic], zi = z[ic];
+        Acc64 acc = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        int n_lo = 0, n_hi = 0, fast_lo = 0, fast_hi = 0;      // inside-cutoff pairs / fast tiles below and above A
+        for (int B = 0; B < nblk; ++B) {
+            const int j0 = B << 5;
+            if (B == A || (ragged && B == nblk - 1)) {
+                tile16<kEnergy, true, true>(x, y, z, j0, ic, N, xi, yi, zi, E, zero, acc, n_lo);
+                tile16<kEnergy, true, true>(x, y, z, j0 + 16, ic, N, xi, yi, zi, E, zero, acc, n_lo);
+            } else if (B > A) {
+                tile16<kEnergy, true, false>(x, y, z, j0, ic, N, xi, yi, zi, E, zero, acc, n_hi);
+                tile16<kEnergy, true, false>(x, y, z, j0 + 16, ic, N, xi, yi, zi, E, zero, acc, n_hi);
+                ++fast_hi;
+            } else {
+                tile16<kEnergy, false, false>(x, y, z, j0, ic, N, xi, yi, zi, E, zero, acc, n_lo);
+                tile16<kEnergy, false, false>(x, y, z, j0 + 16, ic, N, xi, yi, zi, E, zero, acc, n_lo);
+                ++fast_lo;
+            }
+        }
+        if (live) {
+            sv.S[(size_t)w * ld + i] = acc.s;                          // R17: rebuild the running sum
+            if (kEnergy) {
+                const double out_hi = (double)(32 * fast_hi - n_hi), out_all = (double)(32 * (fast_lo + fast_hi) - n_lo - n_hi);
+                tLam += acc.lam - 3840.0 * out_all;
+                tG2 += acc.gx * acc.gx + acc.gy * acc.gy + acc.gz * acc.gz;
+                tV += acc.v - (double)KV * out_hi;
+            }
+        }
+    }
+
+    if (kEnergy) {
+        tLam = warp_sum(tLam); tG2 = warp_sum(tG2); tV = warp_sum(tV);
+        if (lane == 0) { red[warp] = tLam; red[32 + warp] = tG2; red[64 + warp] = tV; }
+        __syncthreads();
+        if (warp == 0) {
+            double a = lane < nwarps ? red[lane] : 0.0;
+            double b = lane < nwarps ? red[32 + lane] : 0.0;
+            double c = lane < nwarps ? red[64 + lane] : 0.0;
+            a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+            if (lane == 0) {
+                // box units -> Angstrom: gradients per box edge; the minimum image carried a factor 2^32
+                const double Dku = Dk * g.inv_unit * g.inv_unit;
+                const double lam = -g.b5 * a;                                  // sum_i Lambda_i
+                const double g2 = (2.5 * g.b5 * 0x1p-32) * (2.5 * g.b5 * 0x1p-32) * b;   // sum_i |G_i|^2
+                const double T_PB = -Dku * (lam + g2);
+                const double T_JF = -0.5 * Dku * lam;
+                double *o = out + (size_t)w * 4;
+                o[0] = c + T_PB; o[1] = c; o[2] = T_PB; o[3] = T_JF;
+            }
+        }
+    }
+}
+
+int smem_bytes32(int N) { return 96 * 8 + 3 * (((N + 31) >> 5) << 5) * 4; }
+
+template <int T>
+cudaError_t launch32(qmc_ctx *c, double *d_out, bool energy)
+{
+    const int smem = smem_bytes32(c->p.N);
+    cudaError_t e;
+    if (energy) {
+        auto k = energy32_kernel<T, true>;
+        if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
+        k<<<c->W, T, smem, c->stream>>>(c->sv, c->p.hbar2_over_2m, d_out);
+    } else {
+        auto k = energy32_kernel<T, false>;
+        if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
+        k<<<c->W, T, smem, c->stream>>>(c->sv, c->p.hbar2_over_2m, d_out);
+    }
+    return cudaGetLastError();
+}
+
+template <int T>
+int occupancy32(int smem)
+{
+    int occ = 0;
+    auto k = energy32_kernel<T, true>;
+    cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, T, smem);
+    return occ;
+}
+
+}  // namespace
+
+#define QMC_E32_THREADS(X) X(32) X(64) X(128) X(256) X(512)
+
+cudaError_t launch_energy_f32(qmc_ctx *c, double *d_out, bool energy)
+{
+    const int T = c->energy_plan.threads;
+#define X(TT) if (T == TT) return launch32<TT>(c, d_out, energy);
+    QMC_E32_THREADS(X)
+#undef X
+    return cudaErrorInvalidValue;
+}
+
+// One warp per 32 particles up to 8 warps; QMC_ENERGY_THREADS overrides (tuning experiments).
+bool plan_energy_f32(qmc_ctx *c, EnergyPlan *out)
+{
+    const int N = c->p.N;
+    int T = 32;
+    while (T < N && T < 256) T *= 2;
+    if (const char *env = getenv("QMC_ENERGY_THREADS")) {
+        const int v = atoi(env);
+        if (v >= 32 && v <= 512 && (v & (v - 1)) == 0) T = v;
+    }
+    out->threads = T;
+    out->smem_bytes = smem_bytes32(N);
+    if (out->smem_bytes > 227 * 1024) return false;
+    out->ctas_per_sm = 0;
+#define X(TT) if (T == TT) out->ctas_per_sm = occupancy32<TT>(out->smem_bytes);
+    QMC_E32_THREADS(X)
+#undef X
+    return true;
+}
+
+}  // namespace qmc

@@ -69,5 +69,7 @@ cudaError_t launch_get_positions(qmc_ctx *c, double *d_xyz);
 cudaError_t launch_acceptance(qmc_ctx *c, double *d_out);
 bool plan_sweep(qmc_ctx *c, SweepPlan *out);
 bool plan_energy(qmc_ctx *c, EnergyPlan *out);
+cudaError_t launch_energy_f32(qmc_ctx *c, double *d_out, bool energy);
+bool plan_energy_f32(qmc_ctx *c, EnergyPlan *out);
 
 }  // namespace qmc

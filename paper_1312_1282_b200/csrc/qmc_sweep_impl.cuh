@@ -28,6 +28,7 @@
 // (l.325), exactly; one I2FP gives it as fp32.  Everything after that is fp32 in box units.
 #pragma once
 #include "qmc_internal.h"
+#include "qmc_f32c.cuh"
 
 namespace qmc {
 
@@ -42,12 +43,6 @@ template <typename Real> struct MoveRand { double logxi; typename ModeT<Real>::D
 
 // V consecutive values as one shared-memory vector access.
 template <typename E, int V> struct alignas(sizeof(E) * V) Pack { E v[V]; };
-
-// ---- FP32C coordinate codec: fp32 s in [1,2)  <->  fixed point (mantissa << 9) -------------------
-__device__ __forceinline__ int32_t enc_coord(float s) { return (int32_t)((__float_as_uint(s) & 0x7FFFFFu) << 9); }
-__device__ __forceinline__ float dec_coord(int32_t k) { return __uint_as_float(0x3F800000u | ((uint32_t)k >> 9)); }
-__device__ __forceinline__ int32_t wsub(int32_t a, int32_t b) { return (int32_t)((uint32_t)a - (uint32_t)b); }
-__device__ __forceinline__ int32_t wadd(int32_t a, int32_t b) { return (int32_t)((uint32_t)a + (uint32_t)b); }
 
 // ---- per-mode constants of the pair function -----------------------------------------------------
 template <typename Real> struct SweepConst;
@@ -96,25 +91,16 @@ __device__ __forceinline__ float pair_t(int32_t px, int32_t py, int32_t pz, int3
     return fmaf(z4, z, fmaf(y4, y, -64.0f));
 }
 
-// ---- packed fp32 (Blackwell FFMA2 / FMUL2 / FADD2: two fp32 lanes per 64-bit register pair, one issue slot) ----
-typedef unsigned long long f32x2;
-__device__ __forceinline__ f32x2 pk2(float a, float b) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
-__device__ __forceinline__ void upk2(f32x2 r, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(r)); }
-__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
-__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
-__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
-
 // Two FP32C pair terms at once: same arithmetic as pair_t(int...) but r^2 stays scaled by 2^64 up to the
 // reciprocal square root (y' = y 2^-32, q = r 2^32), which saves the scaling multiply; the clamp is at
 // 2^62 = h^2 2^64 and bias2 holds 0 or 2^63 per lane (padding).  Every power of two is exact, so the
 // results are bit-identical to the scalar form.
 __device__ __forceinline__ f32x2 pair_t2(int32_t px, int32_t py, int32_t pz, int32_t X0, int32_t X1, int32_t Y0, int32_t Y1,
-                                         int32_t Z0, int32_t Z1, f32x2 bias2)
+                                         int32_t Z0, int32_t Z1, f32x2 bias2, int32_t zero)
 {
-    const f32x2 mx = pk2(__int2float_rn(wsub(px, X0)), __int2float_rn(wsub(px, X1)));
-    const f32x2 my = pk2(__int2float_rn(wsub(py, Y0)), __int2float_rn(wsub(py, Y1)));
-    const f32x2 mz = pk2(__int2float_rn(wsub(pz, Z0)), __int2float_rn(wsub(pz, Z1)));
+    const f32x2 mx = pk2(__int2float_rn(wsub3(px, X0, zero)), __int2float_rn(wsub3(px, X1, zero)));
+    const f32x2 my = pk2(__int2float_rn(wsub3(py, Y0, zero)), __int2float_rn(wsub3(py, Y1, zero)));
+    const f32x2 mz = pk2(__int2float_rn(wsub3(pz, Z0, zero)), __int2float_rn(wsub3(pz, Z1, zero)));
     const f32x2 r2p = fma2(mx, mx, fma2(my, my, fma2(mz, mz, bias2)));
     float a, b;
     upk2(r2p, a, b);
@@ -161,20 +147,20 @@ __device__ __forceinline__ int s_index(int j)
     return ((gi * (V / 2) + (e >> 1)) * T + tid) * 2 + (e & 1);
 }
 
-static inline int sweep_smem_bytes(int T, int J, int mode)
+static inline int sweep_smem_bytes(int T, int J, int mode, int P)
 {
     const int real = (mode == QMC_FP64) ? 8 : 4;
     const int NP = T * J;
-    return NP * 8 + 2 * kChunk * 32 + 64 * 8 + 3 * NP * real;
+    return NP * 8 + 2 * kChunk * 32 + 64 * 8 + 3 * NP * real + (P ? NP * 4 : 0);
 }
 
 // Resident CTAs per SM the register allocator should leave room for: what shared memory allows for
 // this (T,J), capped so that fp64 code keeps >= ~80 and fp32 code >= ~48 registers plus the J retained terms.
-template <typename Real, int T, int J>
+template <typename Real, int T, int J, int P>
 constexpr int sweep_min_ctas()
 {
     const int real = (int)sizeof(Real);
-    const int smem = J * T * (8 + 3 * real) + 2 * kChunk * 32 + 64 * 8 + 1024;
+    const int smem = J * T * (8 + 3 * real + (P ? 4 : 0)) + 2 * kChunk * 32 + 64 * 8 + 1024;
     const int by_smem = (228 * 1024) / smem;
     const int regs = (real == 8 ? 96 + 3 * J : 40 + 3 * J);
     const int by_regs = 65536 / (regs * T);
@@ -205,11 +191,18 @@ __device__ __forceinline__ double sum_parts(const double *pb)
 
 // T threads per CTA; each thread owns J particles in G = J/V packs of V consecutive ones:
 // particle j = (g*T + tid)*V + e, g < G, e < V.  Shared arrays are padded to NP = T*J entries.
-template <typename Real, int T, int J, int V>
-__global__ void __launch_bounds__(T, (sweep_min_ctas<Real, T, J>()))
+// P = 1 (FP32C, V >= 2): the changes t_new - t_old of the running pair sums are first collected in an fp32
+// array `pend` and folded into the fp64 sums S every kFold moves (R20: at most kFold accepted moves, i.e.
+// <= 16 fp32 terms, are summed in fp32 before they reach the fp64 accumulator) -- this takes the
+// fp32 -> fp64 conversions, which run at 1/8 rate, off the per-pair path of an accepted move.
+constexpr int kFold = 16;
+template <typename Real, int T, int J, int V, int PD>
+__global__ void __launch_bounds__(T, (sweep_min_ctas<Real, T, J, PD>()))
 sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
 {
     static_assert(J % V == 0, "J must be a multiple of the vector width");
+    static_assert(PD == 0 || (sizeof(Real) == 4 && V >= 2), "pending sums exist only in the packed FP32C path");
+    constexpr bool kPend = (PD != 0);
     static_assert(V == 1 || V == 2 || V == 4, "vector width");
     using Coord = typename ModeT<Real>::Coord;
     using PackC = Pack<Coord, V>;
@@ -226,6 +219,7 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
     double         *part = reinterpret_cast<double *>(smem_raw + NP * 8 + 2 * kChunk * 32);   // [2][32]
     Coord          *x    = reinterpret_cast<Coord *>(part + 64);                              // [3][NP]
     Coord *y = x + NP, *z = x + 2 * NP;
+    float *pend = reinterpret_cast<float *>(x + 3 * NP);                                      // [NP] (P = 1 only)
     static_assert(sizeof(MoveRand<Real>) <= 32, "variate record must fit its 32-byte slot");
 
     const GroupDev g = sv.groups[sv.group_of[w]];
@@ -252,6 +246,7 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
         }
         x[j] = cx; y[j] = cy; z[j] = cz;
         S[s_index<T, V>(j)] = s;
+        if constexpr (kPend) pend[j] = 0.0f;
     }
 
     // per-pack clamp bias of this thread (FP32C): 1 for padding packs.  Requires N % V == 0 (planner).
@@ -290,7 +285,9 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
         return *reinterpret_cast<const MoveRand<Real> *>(rnd + ((int)((m >> 5) & 1) * kChunk + (int)(m & (kChunk - 1))) * 32);
     };
     produce(0, 0);
+    if (tid == 0) *reinterpret_cast<int32_t *>(part + 63) = 0;
     __syncthreads();
+    const int32_t zero = opaque_zero(reinterpret_cast<int32_t *>(part + 63));   // part[32..63] is used from move 1 on
 
     unsigned long long n_acc = 0;
     int s = 0;
@@ -325,7 +322,7 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
                 const PackC Z = *reinterpret_cast<const PackC *>(z + base);
 #pragma unroll
                 for (int e = 0; e < V; e += 2) {
-                    const f32x2 t2 = pair_t2(tx, ty, tz, X.v[e], X.v[e + 1], Y.v[e], Y.v[e + 1], Z.v[e], Z.v[e + 1], bias2[gi]);
+                    const f32x2 t2 = pair_t2(tx, ty, tz, X.v[e], X.v[e + 1], Y.v[e], Y.v[e + 1], Z.v[e], Z.v[e + 1], bias2[gi], zero);
                     un2[(gi * V + e) / 2] = t2;
                     acc2 = add2(acc2, t2);
                 }
@@ -348,7 +345,11 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
             }
         }
         double acc = (double)accr;
-        if (owner) acc -= S[s_index<T, V>(s)];             // a4: sum_j t_new - S_s
+        if (owner) {                                       // a4: sum_j t_new - S_s
+            double Ss = S[s_index<T, V>(s)];
+            if constexpr (kPend) Ss += (double)pend[s];
+            acc -= Ss;
+        }
 
         // a5: block sum, identical bits in every thread
         double tot = warp_sum(acc);
@@ -387,6 +388,17 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
                 if constexpr (V == 1) {
                     const Real to = pair_t(xs, ys, zs, X.v[0], Y.v[0], Z.v[0], bias[gi], P);
                     S[base] += (double)(un[gi] - to);
+                } else if constexpr (kPend) {
+                    using PackF = Pack<float, V>;
+                    PackF pd = *reinterpret_cast<const PackF *>(pend + base);
+#pragma unroll
+                    for (int c = 0; c < V / 2; ++c) {
+                        const f32x2 to2 = pair_t2(xs, ys, zs, X.v[2 * c], X.v[2 * c + 1], Y.v[2 * c], Y.v[2 * c + 1],
+                                                  Z.v[2 * c], Z.v[2 * c + 1], bias2[gi], zero);
+                        const f32x2 nw = add2(pk2(pd.v[2 * c], pd.v[2 * c + 1]), sub2(un2[(gi * V) / 2 + c], to2));
+                        upk2(nw, pd.v[2 * c], pd.v[2 * c + 1]);
+                    }
+                    *reinterpret_cast<PackF *>(pend + base) = pd;
                 } else {
 #pragma unroll
                     for (int c = 0; c < V / 2; ++c) {
@@ -394,7 +406,7 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
                         double2 sv2 = *sp;
                         if constexpr (kPacked) {
                             const f32x2 to2 = pair_t2(xs, ys, zs, X.v[2 * c], X.v[2 * c + 1], Y.v[2 * c], Y.v[2 * c + 1],
-                                                      Z.v[2 * c], Z.v[2 * c + 1], bias2[gi]);
+                                                      Z.v[2 * c], Z.v[2 * c + 1], bias2[gi], zero);
                             float d0, d1;
                             upk2(sub2(un2[(gi * V) / 2 + c], to2), d0, d1);
                             sv2.x += (double)d0;
@@ -410,7 +422,8 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
                 }
             }
             if (owner) {
-                S[s_index<T, V>(s)] += tot;
+                if constexpr (kPend) { S[s_index<T, V>(s)] += (double)pend[s] + tot; pend[s] = 0.0f; }
+                else                 S[s_index<T, V>(s)] += tot;
                 x[s] = commit_coord(tx, g.L);
                 y[s] = commit_coord(ty, g.L);
                 z[s] = commit_coord(tz, g.L);
@@ -418,6 +431,27 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
             ++n_acc;
         } else if (owner) {
             x[s] = xs;                                      // undo the poison
+        }
+        if constexpr (kPend) {
+            if ((m & (kFold - 1)) == kFold - 1 || m + 1 == total) {       // fold the pending changes into S
+#pragma unroll
+                for (int gi = 0; gi < G; ++gi) {
+                    using PackF = Pack<float, V>;
+                    const int base = (gi * T + tid) * V;
+                    const PackF pd = *reinterpret_cast<const PackF *>(pend + base);
+                    PackF zr;
+#pragma unroll
+                    for (int c = 0; c < V / 2; ++c) {
+                        double2 *sp = reinterpret_cast<double2 *>(S + ((gi * (V / 2) + c) * T + tid) * 2);
+                        double2 sv2 = *sp;
+                        sv2.x += (double)pd.v[2 * c];
+                        sv2.y += (double)pd.v[2 * c + 1];
+                        *sp = sv2;
+                        zr.v[2 * c] = 0.0f; zr.v[2 * c + 1] = 0.0f;
+                    }
+                    *reinterpret_cast<PackF *>(pend + base) = zr;
+                }
+            }
         }
         s = sn;
         xs = xn; ys = yn; zs = zn;
@@ -440,33 +474,33 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
 
 // ---- host side: one table entry per compiled (T, J, V) shape ----------------------------------------
 struct SweepShape {
-    int T, J, V;
+    int T, J, V, P;
     cudaError_t (*launch)(qmc_ctx *c, int n_sweeps, int smem);
     int (*occupancy)(int smem);
 };
 
-template <typename Real, int T, int J, int V>
+template <typename Real, int T, int J, int V, int PD>
 static cudaError_t shape_launch(qmc_ctx *c, int n_sweeps, int smem)
 {
     const uint2 key = make_uint2((uint32_t)(c->seed & 0xFFFFFFFFull), (uint32_t)(c->seed >> 32));
-    auto kern = sweep_kernel<Real, T, J, V>;
+    auto kern = sweep_kernel<Real, T, J, V, PD>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     kern<<<c->W, T, smem, c->stream>>>(c->sv, c->trace, key, c->t, n_sweeps);
     return cudaGetLastError();
 }
 
-template <typename Real, int T, int J, int V>
+template <typename Real, int T, int J, int V, int PD>
 static int shape_occupancy(int smem)
 {
     int n = 0;
-    auto kern = sweep_kernel<Real, T, J, V>;
+    auto kern = sweep_kernel<Real, T, J, V, PD>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, T, smem) != cudaSuccess) return 0;
     return n;
 }
 
-#define QMC_SHAPE_ENTRY(Real, TT, JJ, VV) {TT, JJ, VV, shape_launch<Real, TT, JJ, VV>, shape_occupancy<Real, TT, JJ, VV>},
+#define QMC_SHAPE_ENTRY(Real, TT, JJ, VV, PP) {TT, JJ, VV, PP, shape_launch<Real, TT, JJ, VV, PP>, shape_occupancy<Real, TT, JJ, VV, PP>},
 
 const SweepShape *sweep_shapes_f32(int *n);
 const SweepShape *sweep_shapes_f64(int *n);

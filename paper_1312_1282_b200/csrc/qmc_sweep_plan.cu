@@ -15,7 +15,7 @@ cudaError_t launch_sweep(qmc_ctx *c, int n_sweeps)
 }
 
 // Threads per walker the heuristic aims at: about 16 particles per thread (measured on B200, profiles/),
-// one warp at least.  QMC_SWEEP_SHAPE="T,J[,V]" overrides the heuristic (tuning experiments).
+// one warp at least.  QMC_SWEEP_SHAPE="T,J[,V[,P]]" overrides the heuristic (tuning experiments).
 bool plan_sweep(qmc_ctx *c, SweepPlan *out)
 {
     const int N = c->p.N, mode = c->p.mode;
@@ -24,15 +24,15 @@ bool plan_sweep(qmc_ctx *c, SweepPlan *out)
     auto usable = [&](const SweepShape &s) {
         if ((long long)s.T * s.J < N) return false;
         if (s.V > 1 && N % s.V != 0) return false;
-        return sweep_smem_bytes(s.T, s.J, mode) <= 227 * 1024;
+        return sweep_smem_bytes(s.T, s.J, mode, s.P) <= 227 * 1024;
     };
     const SweepShape *best = nullptr;
     if (const char *env = getenv("QMC_SWEEP_SHAPE")) {
-        int t = 0, j = 0, v = 0;
-        const int got = sscanf(env, "%d,%d,%d", &t, &j, &v);
+        int t = 0, j = 0, v = 0, pp = 0;
+        const int got = sscanf(env, "%d,%d,%d,%d", &t, &j, &v, &pp);
         for (int k = 0; k < n && got >= 2; ++k)
-            if (tab[k].T == t && tab[k].J == j && (got < 3 || tab[k].V == v) && usable(tab[k]))
-                if (!best || tab[k].V > best->V) best = &tab[k];
+            if (tab[k].T == t && tab[k].J == j && (got < 3 || tab[k].V == v) && (got < 4 || tab[k].P == pp) && usable(tab[k]))
+                if (!best || tab[k].V > best->V || (tab[k].V == best->V && tab[k].P > best->P)) best = &tab[k];
     }
     if (!best) {
         const int per_thread = 16;
@@ -42,7 +42,7 @@ bool plan_sweep(qmc_ctx *c, SweepPlan *out)
             if (!usable(tab[k])) continue;
             const double waste = (double)(tab[k].T * tab[k].J - N) / (double)N;       // idle slots
             const double score = 4.0 * waste + std::fabs(std::log2((double)tab[k].T) - t_target)
-                               + (mode == QMC_FP64 ? 0.25 * (2 - tab[k].V) : 0.25 * (4 - tab[k].V));
+                               + (mode == QMC_FP64 ? 0.25 * (2 - tab[k].V) : 0.25 * (4 - tab[k].V)) - 0.1 * tab[k].P;
             if (score < best_score) { best_score = score; best = &tab[k]; }
         }
     }
@@ -50,7 +50,7 @@ bool plan_sweep(qmc_ctx *c, SweepPlan *out)
     out->smem_bytes = N * (8 + 3 * (mode == QMC_FP64 ? 8 : 4));
     if (!best) return false;
     out->threads = best->T; out->J = best->J; out->V = best->V; out->shape = best;
-    out->smem_bytes = sweep_smem_bytes(best->T, best->J, mode);
+    out->smem_bytes = sweep_smem_bytes(best->T, best->J, mode, best->P);
     out->ctas_per_sm = best->occupancy(out->smem_bytes);
     return true;
 }
