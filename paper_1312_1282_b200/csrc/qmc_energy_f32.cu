@@ -9,13 +9,13 @@
 // instruction: all pair arithmetic is packed f32x2.
 //
 //   G_i      = sum_{j != i} u'(r_ij) d_ij / r_ij,     u'/r = 5/2 b^5 y (y^6 - z^6)
-//   Lambda_i = sum_{j != i} [u'' + 2 u'/r]                 = -b^5 (10 y^7 + z^6 (15 z + 5 y))
+//   Lambda_i = sum_{j != i} [u'' + 2 u'/r]                 = -5 b^5 (2 y^7 + 3 z^7 + z^6 y)
 //   V        = sum_{i<j, r<h} V_Aziz(r_ij)                 (HFD-B(HE), truncated at h, R3)
 //   T_PB = -Dk sum_i (Lambda_i + |G_i|^2),  T_JF = -Dk/2 sum_i Lambda_i,  E_PB = V + T_PB      (R14)
 // with y = 1/r, z = 1/(L-r), box units (L = 1, h = 1/2).
 //
 // No per-pair cutoff test.  r^2 is CLAMPED to h^2, where y = z = 2 exactly, so a pair at or beyond the
-// cutoff contributes exactly 0 to S_i and G_i, and exactly the constants K_L = 3840 (lap term) and
+// cutoff contributes exactly 0 to S_i and G_i, and exactly the constants K_L = 768 (lap term / 5 b^5) and
 // K_V = V(h) to the other two sums; the kernel counts the pairs inside the cutoff (one integer compare) and
 // removes (pairs - inside) K afterwards in fp64.  Only the j-block that contains the warp's own particles
 // (self pair, V for j > i only) and a ragged last block take a slower tile with explicit selects.
@@ -38,13 +38,13 @@ constexpr int   kClampBits = 0x5E800000;       // bit pattern of 2^62
 // or carried as hi + lo, so that no fp32 rounding of a CONSTANT puts a systematic relative error on
 // every pair (the box-unit value of r_m is an arbitrary real number):
 //   rep  = eps A 2^(a1 r + a2 r^2),  a1 = -alpha log2(e) / r_m,  a2 = beta log2(e) / r_m^2   (hi + lo)
-//   disp = w^3 (k6 + w (k8 + w k10)),  w = fl(r_m^2) y^2,  k_n = eps c_n (r_m^2 / fl(r_m^2))^(n/2)
-//   F    = 2^(-log2(e) max(D r_m y - 1, 0)^2)                                     (D r_m hi + lo)
+//   disp = v^3 (k6 + v (k8 + v k10)),  v = y^2,  k_n = eps c_n r_m^n
+//   F    = 2^(-(sqrt(log2 e) max(D r_m y - 1, 0))^2)                              (D r_m hi + lo)
 struct AzizF32 {
-    f32x2 a1h, a1l, a2h, a2l, epsA, epsAln2, rm2, nk6, nk8, nk10, Drm, Drml;
+    f32x2 a1h, a1l, a2h, a2l, epsA, epsAln2, nk6, nk8, nk10, Dh, Dl, nDc;
     __device__ __forceinline__ void load(const AzizDev &a)
     {
-        const double log2e = 1.4426950408889634, ln2 = 0.6931471805599453;
+        const double log2e = 1.4426950408889634, ln2 = 0.6931471805599453, sl = 1.2011224087864498;   // sqrt(log2 e)
         auto split = [](double v, f32x2 &hi, f32x2 &lo) {
             const float h = __double2float_rn(v);
             hi = pk1(h);
@@ -55,24 +55,22 @@ struct AzizF32 {
         const float eA = (float)(a.eps * a.A);
         epsA = pk1(eA);
         epsAln2 = pk1((float)((double)eA * ln2));
-        const float rm2f = (float)a.rm2;
-        rm2 = pk1(rm2f);
-        const double q = a.rm2 / (double)rm2f;            // 1 + rounding error of fl(r_m^2)
-        nk6 = pk1((float)(-a.eps * a.c6 * q * q * q));
-        nk8 = pk1((float)(-a.eps * a.c8 * q * q * q * q));
-        nk10 = pk1((float)(-a.eps * a.c10 * q * q * q * q * q));
-        split(a.Drm, Drm, Drml);
+        const double r2 = a.rm2, r6 = r2 * r2 * r2;
+        nk6 = pk1((float)(-a.eps * a.c6 * r6));
+        nk8 = pk1((float)(-a.eps * a.c8 * r6 * r2));
+        nk10 = pk1((float)(-a.eps * a.c10 * r6 * r2 * r2));
+        split(a.Drm * sl, Dh, Dl);
+        nDc = pk1((float)(-sl));
     }
 };
 
 // Everything the pair arithmetic of two j produces.
 struct Pair2 {
     f32x2 mx, my, mz;      // signed minimum image, 2^32 box units
-    f32x2 r2c;             // min(r^2, h^2) 2^64
     f32x2 yp, q;           // y 2^-32 (hardware rsqrt), r 2^32
     f32x2 y, z;            // 1/r, 1/(1-r)
     f32x2 y2, z2, y4, z4;
-    float a, b;            // the two lanes of r2c
+    float a, b;            // the two lanes of min(r^2, h^2) 2^64
 };
 
 __device__ __forceinline__ Pair2 pair_geom(int32_t xi, int32_t yi, int32_t zi, int32_t X0, int32_t X1, int32_t Y0, int32_t Y1,
@@ -86,9 +84,8 @@ __device__ __forceinline__ Pair2 pair_geom(int32_t xi, int32_t yi, int32_t zi, i
     upk2(r2p, p.a, p.b);
     p.a = fminf(p.a, kClamp);
     p.b = fminf(p.b, kClamp);
-    p.r2c = pk2(p.a, p.b);
     p.yp = pk2(rsqrt_pos(p.a), rsqrt_pos(p.b));
-    p.q = mul2(p.r2c, p.yp);
+    p.q = mul2(pk2(p.a, p.b), p.yp);
     const f32x2 omr = fma2(p.q, pk1(-0x1p-32f), pk1(1.0f));
     float oa, ob;
     upk2(omr, oa, ob);
@@ -104,48 +101,52 @@ __device__ __forceinline__ Pair2 pair_geom(int32_t xi, int32_t yi, int32_t zi, i
 // t = y^5 + z^5 - 64 (raw pair-sum term, u = c1 t); exactly 0 at the clamp
 __device__ __forceinline__ f32x2 pair_t(const Pair2 &p) { return fma2(p.z4, p.z, fma2(p.y4, p.y, pk1(-64.0f))); }
 
-// HFD-B(HE) of the two pairs in K.  The hardware rsqrt is first refined by one Newton step (the seed is
-// good to ~2^-22 and the repulsive exponential amplifies a relative error of r ~11x).
+// HFD-B(HE) of the two pairs in K.  The hardware rsqrt is first refined by one Newton step,
+// y = y0 f with f = 3/2 - r^2 y0^2 / 2 (the seed is good to ~2^-22 and the repulsive exponential
+// amplifies a relative error of r ~11x); r = r^2 y0 f.
 __device__ __forceinline__ f32x2 aziz2(const Pair2 &p, const AzizF32 &E)
 {
-    const f32x2 e = fma2(mul2(p.q, pk1(-1.0f)), p.yp, pk1(1.0f));          // 1 - r^2 y0^2
-    const f32x2 y = fma2(mul2(p.y, pk1(0.5f)), e, p.y);
-    const f32x2 r = mul2(mul2(p.r2c, pk1(0x1p-64f)), y);
-    const f32x2 w = mul2(E.rm2, mul2(y, y));
-    const f32x2 w3 = mul2(mul2(w, w), w);
-    const f32x2 ndisp = mul2(w3, fma2(w, fma2(w, E.nk10, E.nk8), E.nk6));   // -disp
-    const f32x2 t = fma2(E.Drml, y, fma2(E.Drm, y, pk1(-1.0f)));           // D/x - 1
+    const f32x2 f = fma2(p.q, mul2(p.yp, pk1(-0.5f)), pk1(1.5f));
+    const f32x2 y = mul2(p.y, f);
+    const f32x2 r = mul2(mul2(p.q, pk1(0x1p-32f)), f);
+    const f32x2 v = mul2(y, y);
+    const f32x2 v3 = mul2(mul2(v, v), v);
+    const f32x2 ndisp = mul2(v3, fma2(v, fma2(v, E.nk10, E.nk8), E.nk6));   // -disp
+    const f32x2 t = fma2(E.Dl, y, fma2(E.Dh, y, E.nDc));                    // sqrt(log2 e) (D/x - 1)
     float ta, tb;
     upk2(t, ta, tb);
-    const f32x2 tc = pk2(fmaxf(ta, 0.0f), fmaxf(tb, 0.0f));                // F = 1 for x >= D
-    const f32x2 fa = mul2(mul2(tc, tc), pk1(-1.4426950408889634f));
+    const f32x2 tc = pk2(fmaxf(ta, 0.0f), fmaxf(tb, 0.0f));                 // F = 1 for x >= D
     float f0, f1;
-    upk2(fa, f0, f1);
-    const f32x2 F = pk2(ex2_approx(f0), ex2_approx(f1));
+    upk2(mul2(tc, tc), f0, f1);
+    const f32x2 F = pk2(ex2_approx(-f0), ex2_approx(-f1));
     const f32x2 t1 = fma2(E.a2h, r, E.a1h);
     const f32x2 ah = mul2(r, t1);
-    f32x2 al = fma2(r, t1, mul2(ah, pk1(-1.0f)));                          // exact residual of the product
-    al = fma2(r, fma2(E.a2l, r, E.a1l), al);
-    float h0, h1;
+    float r0, r1, t10, t11, h0, h1;
+    upk2(r, r0, r1);
+    upk2(t1, t10, t11);
     upk2(ah, h0, h1);
+    f32x2 al = pk2(fmaf(r0, t10, -h0), fmaf(r1, t11, -h1));                 // exact residual of the product
+    al = fma2(r, fma2(E.a2l, r, E.a1l), al);
     const f32x2 e2 = pk2(ex2_approx(h0), ex2_approx(h1));
-    const f32x2 rep = fma2(mul2(e2, E.epsAln2), al, mul2(e2, E.epsA));     // eps A 2^ah (1 + ln2 al)
+    const f32x2 rep = mul2(e2, fma2(al, E.epsAln2, E.epsA));                // eps A 2^ah (1 + ln2 al)
     return fma2(F, ndisp, rep);
 }
 
 struct Acc32 { f32x2 gx, gy, gz, lam, s, v; };
-struct Acc64 { double gx, gy, gz, lam, s, v; };
+struct Acc64 { double gx, gy, gz, lam, lamd, s, v; };   // lam: tiles above the diagonal (counted twice), lamd: diagonal tile
 
 // 16 consecutive j (4 vector loads per coordinate) against this lane's particle.
-//   kSlow: per-pair selects (self pair, j >= N, V only for j > i); kV: evaluate the potential.
+//   kSlow: per-pair selects (self pair, j >= N, V only for j > i); kV: evaluate the potential and the
+//   Laplacian term (both are symmetric in i,j and only their totals are needed: tiles below the diagonal skip them).
+// Sums kept here: gm = y^7 - z^6 y = (u'/r) / (5/2 b^5);  lt = 2 y^7 + 3 z^7 + z^6 y = -(u'' + 2u'/r) / (5 b^5).
 template <bool kEnergy, bool kV, bool kSlow>
 __device__ __forceinline__ void tile16(const int32_t *__restrict__ x, const int32_t *__restrict__ y, const int32_t *__restrict__ z,
                                        int j0, int i, int N, int32_t xi, int32_t yi, int32_t zi, const AzizF32 &E,
-                                       int32_t zero, Acc64 &A, int &n_in)
+                                       int32_t zero, Acc64 &A, double &lam_acc, int &n_in)
 {
     Acc32 P;
     P.gx = P.gy = P.gz = P.lam = P.s = P.v = pk1(0.0f);
-#pragma unroll
+#pragma unroll 1
     for (int g = 0; g < 4; ++g) {
         const int4 X = *reinterpret_cast<const int4 *>(x + j0 + 4 * g);
         const int4 Y = *reinterpret_cast<const int4 *>(y + j0 + 4 * g);
@@ -161,22 +162,22 @@ __device__ __forceinline__ void tile16(const int32_t *__restrict__ x, const int3
             P.s = add2(P.s, pair_t(p));
             if (kEnergy) {
                 const f32x2 y6 = mul2(p.y4, p.y2), z6 = mul2(p.z4, p.z2);
-                const f32x2 gm = mul2(p.y, sub2(y6, z6));                                    // (u'/r) / (5/2 b^5)
+                const f32x2 y7 = mul2(y6, p.y), z6y = mul2(z6, p.y);
+                const f32x2 z7 = kV ? mul2(z6, p.z) : z6;
+                const f32x2 gm = sub2(y7, z6y);
                 P.gx = fma2(gm, p.mx, P.gx);
                 P.gy = fma2(gm, p.my, P.gy);
                 P.gz = fma2(gm, p.mz, P.gz);
-                const f32x2 y7 = mul2(y6, p.y);
-                const f32x2 inner = fma2(p.z, pk1(15.0f), mul2(p.y, pk1(5.0f)));
-                f32x2 lt = fma2(y7, pk1(10.0f), mul2(z6, inner));                            // -(u'' + 2u'/r) / b^5
-                if (kSlow) {
-                    float la, lb;
-                    upk2(lt, la, lb);
-                    lt = pk2(ina ? la : 0.0f, inb ? lb : 0.0f);
-                } else {
-                    n_in += (ina ? 1 : 0) + (inb ? 1 : 0);
-                }
-                P.lam = add2(P.lam, lt);
                 if (kV) {
+                    f32x2 lt = fma2(y7, pk1(2.0f), fma2(z7, pk1(3.0f), z6y));
+                    if (kSlow) {
+                        float la, lb;
+                        upk2(lt, la, lb);
+                        lt = pk2(ina ? la : 0.0f, inb ? lb : 0.0f);
+                    } else {
+                        n_in += (ina ? 1 : 0) + (inb ? 1 : 0);
+                    }
+                    P.lam = add2(P.lam, lt);
                     f32x2 vp = aziz2(p, E);
                     if (kSlow) {
                         float va, vb;
@@ -193,8 +194,10 @@ __device__ __forceinline__ void tile16(const int32_t *__restrict__ x, const int3
         A.gx += (double)hsum2(P.gx);
         A.gy += (double)hsum2(P.gy);
         A.gz += (double)hsum2(P.gz);
-        A.lam += (double)hsum2(P.lam);
-        if (kV) A.v += (double)hsum2(P.v);
+        if (kV) {
+            lam_acc += (double)hsum2(P.lam);
+            A.v += (double)hsum2(P.v);
+        }
     }
 }
 
@@ -244,28 +247,28 @@ energy32_kernel(StateView sv, double Dk, double *__restrict__ out)
         const bool live = i < N;
         const int ic = live ? i : N - 1;
         const int32_t xi = x[ic], yi = y[ic], zi = z[ic];
-        Acc64 acc = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-        int n_lo = 0, n_hi = 0, fast_lo = 0, fast_hi = 0;      // inside-cutoff pairs / fast tiles below and above A
+        Acc64 acc = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        int n_hi = 0, fast_hi = 0, n_none = 0;                 // inside-cutoff pairs / fast tiles above A
         for (int B = 0; B < nblk; ++B) {
             const int j0 = B << 5;
             if (B == A || (ragged && B == nblk - 1)) {
-                tile16<kEnergy, true, true>(x, y, z, j0, ic, N, xi, yi, zi, E, zero, acc, n_lo);
-                tile16<kEnergy, true, true>(x, y, z, j0 + 16, ic, N, xi, yi, zi, E, zero, acc, n_lo);
+                double &la = (B == A) ? acc.lamd : acc.lam;
+                tile16<kEnergy, true, true>(x, y, z, j0, ic, N, xi, yi, zi, E, zero, acc, la, n_none);
+                tile16<kEnergy, true, true>(x, y, z, j0 + 16, ic, N, xi, yi, zi, E, zero, acc, la, n_none);
             } else if (B > A) {
-                tile16<kEnergy, true, false>(x, y, z, j0, ic, N, xi, yi, zi, E, zero, acc, n_hi);
-                tile16<kEnergy, true, false>(x, y, z, j0 + 16, ic, N, xi, yi, zi, E, zero, acc, n_hi);
+                tile16<kEnergy, true, false>(x, y, z, j0, ic, N, xi, yi, zi, E, zero, acc, acc.lam, n_hi);
+                tile16<kEnergy, true, false>(x, y, z, j0 + 16, ic, N, xi, yi, zi, E, zero, acc, acc.lam, n_hi);
                 ++fast_hi;
             } else {
-                tile16<kEnergy, false, false>(x, y, z, j0, ic, N, xi, yi, zi, E, zero, acc, n_lo);
-                tile16<kEnergy, false, false>(x, y, z, j0 + 16, ic, N, xi, yi, zi, E, zero, acc, n_lo);
-                ++fast_lo;
+                tile16<kEnergy, false, false>(x, y, z, j0, ic, N, xi, yi, zi, E, zero, acc, acc.lam, n_none);
+                tile16<kEnergy, false, false>(x, y, z, j0 + 16, ic, N, xi, yi, zi, E, zero, acc, acc.lam, n_none);
             }
         }
         if (live) {
             sv.S[(size_t)w * ld + i] = acc.s;                          // R17: rebuild the running sum
             if (kEnergy) {
-                const double out_hi = (double)(32 * fast_hi - n_hi), out_all = (double)(32 * (fast_lo + fast_hi) - n_lo - n_hi);
-                tLam += acc.lam - 3840.0 * out_all;
+                const double out_hi = (double)(32 * fast_hi - n_hi);
+                tLam += 2.0 * (acc.lam - 768.0 * out_hi) + acc.lamd;
                 tG2 += acc.gx * acc.gx + acc.gy * acc.gy + acc.gz * acc.gz;
                 tV += acc.v - (double)KV * out_hi;
             }
@@ -284,7 +287,7 @@ energy32_kernel(StateView sv, double Dk, double *__restrict__ out)
             if (lane == 0) {
                 // box units -> Angstrom: gradients per box edge; the minimum image carried a factor 2^32
                 const double Dku = Dk * g.inv_unit * g.inv_unit;
-                const double lam = -g.b5 * a;                                  // sum_i Lambda_i
+                const double lam = -5.0 * g.b5 * a;                            // sum_i Lambda_i
                 const double g2 = (2.5 * g.b5 * 0x1p-32) * (2.5 * g.b5 * 0x1p-32) * b;   // sum_i |G_i|^2
                 const double T_PB = -Dku * (lam + g2);
                 const double T_JF = -0.5 * Dku * lam;
