@@ -1,0 +1,291 @@
+// qmc_energy_f64.cu -- FP64 local-energy estimator over all pairs and the
+// from-scratch rebuild of the running pair sums S_i (R17), every UNORDERED pair evaluated once.
+//
+// The fp64 pipe is what bounds this mode (64 lanes per SM, every DFMA/DADD/DMUL two issue cycles), so the
+// kernel spends shuffles, shared-memory traffic and integer work -- all on other pipes -- to halve the
+// fp64 work: the particles are cut into blocks of 32, a warp takes a pair of blocks (A, B), lane l holds
+// particle i = 32A + l AND the accumulators of particle j = 32B + l, and in step s lane l evaluates the pair
+// (i_l, j_{(l+s) mod 32}).  The i-side sums stay in the lane's registers; the j-side terms travel by one
+// indexed shuffle to the lane that holds j.  Block pairs are visited along a ring, B = A + k mod n,
+// k = 1 .. (n-1)/2 (+ half of k = n/2 for even n), the diagonal block with steps 1..16: each pair once.
+// Per-block sums are merged with shared-memory atomics (a few per 1024 pairs).
+//
+//   G_i      = sum_{j != i} u'(r_ij) d_ij / r_ij,     u'/r = 5/2 b^5 (y^7 - z^6 y)
+//   Lambda_i = sum_{j != i} [u'' + 2 u'/r]                 = -5 b^5 (2 y^7 + 3 z^7 + z^6 y)
+//   V        = sum_{i<j, r<h} V_Aziz(r_ij)                 (HFD-B(HE), truncated at h, R3)
+//   T_PB = -Dk sum_i (Lambda_i + |G_i|^2),  T_JF = -Dk/2 sum_i Lambda_i,  E_PB = V + T_PB      (R14)
+// with y = 1/r, z = 1/(L-r).
+//
+// Cutoff: r^2 is clamped to h^2 for the arithmetic (nothing overflows) and the four pair terms of a pair
+// beyond the cutoff, of a padding slot, or of the inactive half of the last diagonal step are selected to
+// exactly 0 -- one DSETP on the fp64 pipe, the selects run on the integer pipe.
+#include "qmc_internal.h"
+
+namespace qmc {
+
+namespace {
+
+struct Const64 {
+    double L, h, h2, sh;
+    double eps, inv_rm, rm2, A, alpha, beta, c6, c8, c10, D, Drm;
+    __device__ __forceinline__ void load(const GroupDev &g)
+    {
+        L = g.L; h = g.h; h2 = g.h2; sh = g.sh;
+        const AzizDev &a = g.az;
+        eps = a.eps; inv_rm = a.inv_rm; rm2 = a.rm2; A = a.A; alpha = a.alpha; beta = a.beta;
+        c6 = a.c6; c8 = a.c8; c10 = a.c10; D = a.D; Drm = a.Drm;
+    }
+};
+
+// signed minimum-image component for |a - b| <= L: magnitude by the fold h - |h - |d||, sign = sign(d)
+// flipped when |d| > h (two integer operations on the high word)
+__device__ __forceinline__ double min_image(double a, double b, double h)
+{
+    const double d = a - b;
+    const double f = h - fabs(d);
+    const double m = h - fabs(f);
+    const int hi = __double2hiint(m) | ((__double2hiint(d) ^ __double2hiint(f)) & 0x80000000);
+    return __hiloint2double(hi, __double2loint(m));
+}
+
+struct Pair64 { double mx, my, mz, t, gm, lt, v; bool in; };
+
+// all terms of one pair; bias > 0 pushes the pair beyond the cutoff
+template <bool kEnergy>
+__device__ __forceinline__ Pair64 pair64(double xi, double yi, double zi, double xs, double ys, double zs,
+                                         double bias, const Const64 &C)
+{
+    Pair64 p;
+    p.mx = min_image(xi, xs, C.h);
+    p.my = min_image(yi, ys, C.h);
+    p.mz = min_image(zi, zs, C.h);
+    const double r2 = fma(p.mz, p.mz, fma(p.my, p.my, fma(p.mx, p.mx, bias)));
+    p.in = r2 < C.h2;
+    const double r2c = p.in ? r2 : C.h2;
+    const double y = rsqrt_pos(r2c);
+    const double r = r2c * y;
+    const double z = rcp_pos(C.L - r);
+    const double y2 = y * y, z2 = z * z;
+    const double y4 = y2 * y2, z4 = z2 * z2;
+    const double t = fma(z4, z, fma(y4, y, -C.sh));
+    p.t = p.in ? t : 0.0;
+    p.gm = 0.0; p.lt = 0.0; p.v = 0.0;
+    if (kEnergy) {
+        const double y6 = y4 * y2, z6 = z4 * z2;
+        const double y7 = y6 * y, z6y = z6 * y, z7 = z6 * z;
+        p.gm = p.in ? y7 - z6y : 0.0;
+        p.lt = p.in ? fma(2.0, y7, fma(3.0, z7, z6y)) : 0.0;
+        const double x = r * C.inv_rm;
+        const double w = C.rm2 * y2;                                // 1/x^2
+        const double disp = w * w * w * fma(w, fma(w, C.c10, C.c8), C.c6);
+        double F = 1.0;
+        if (__any_sync(0xffffffffu, x < C.D)) {
+            const double q = fma(C.Drm, y, -1.0);                   // D/x - 1
+            const double e = exp(-q * q);
+            F = x < C.D ? e : 1.0;
+        }
+        const double rep = C.A * exp(x * fma(C.beta, x, -C.alpha));
+        p.v = p.in ? C.eps * fma(-F, disp, rep) : 0.0;
+    }
+    return p;
+}
+
+__device__ __forceinline__ double shfl_from(double v, int src)
+{
+    return __hiloint2double(__shfl_sync(0xffffffffu, __double2hiint(v), src), __shfl_sync(0xffffffffu, __double2loint(v), src));
+}
+
+template <int T, bool kEnergy>
+__global__ void __launch_bounds__(T)
+energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int N = sv.N, ld = sv.ld;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int nwarps = T >> 5;
+    const int w = blockIdx.x;
+    const int nblk = (N + 31) >> 5, NP = nblk << 5;
+
+    double *red = reinterpret_cast<double *>(smem_raw);               // [3][32]
+    int    *ctr = reinterpret_cast<int *>(red + 96);                  // work counter (+ padding to 16 bytes)
+    double *x   = red + 98;                                           // [3][NP]
+    double *y = x + NP, *z = x + 2 * NP;
+    double *ag = x + 3 * NP;                                          // [4][NP]: G_x, G_y, G_z, S (raw units)
+
+    const GroupDev g = sv.groups[sv.group_of[w]];
+    Const64 C;
+    C.load(g);
+
+    const double *gpos = reinterpret_cast<const double *>(sv.pos) + (size_t)w * 3 * ld;
+    for (int j = tid; j < NP; j += T) {
+        const bool in = j < N;
+        x[j] = in ? gpos[j] : 0.0;
+        y[j] = in ? gpos[ld + j] : 0.0;
+        z[j] = in ? gpos[2 * ld + j] : 0.0;
+        ag[j] = 0.0; ag[NP + j] = 0.0; ag[2 * NP + j] = 0.0; ag[3 * NP + j] = 0.0;
+    }
+    if (tid == 0) *ctr = 0;
+    __syncthreads();
+
+    const double kBig = 4.0 * C.L * C.L;                              // > any r^2: forces the clamp
+
+    const int K = (nblk - 1) >> 1;                                    // full ring offsets
+    const bool even = (nblk & 1) == 0;
+    double tLam = 0.0, tV = 0.0;
+    for (;;) {
+        int A = 0;
+        if (lane == 0) A = atomicAdd(ctr, 1);
+        A = __shfl_sync(0xffffffffu, A, 0);
+        if (A >= nblk) break;
+        const int i = (A << 5) + lane;
+        const bool vi = i < N;
+        const double xi = x[i], yi = y[i], zi = z[i];
+        double gxi = 0.0, gyi = 0.0, gzi = 0.0, si = 0.0;
+        const int kmax = K + ((even && A < (nblk >> 1)) ? 1 : 0);
+        for (int k = 0; k <= kmax; ++k) {
+            int B = A + k;
+            if (B >= nblk) B -= nblk;
+            const int jb = B << 5;
+            const bool vj = jb + lane < N;
+            double gxj = 0.0, gyj = 0.0, gzj = 0.0, sj = 0.0;
+            const int s0 = (k == 0) ? 1 : 0, s1 = (k == 0) ? 17 : 32;
+            for (int s = s0; s < s1; ++s) {
+                const int src = (lane + s) & 31;
+                const bool ok = vi && (jb + src < N) && !(k == 0 && s == 16 && lane >= 16);
+                const Pair64 p = pair64<kEnergy>(xi, yi, zi, x[jb + src], y[jb + src], z[jb + src], ok ? 0.0 : kBig, C);
+                si += p.t;
+                double cx = 0.0, cy = 0.0, cz = 0.0;
+                if (kEnergy) {
+                    cx = p.gm * p.mx; cy = p.gm * p.my; cz = p.gm * p.mz;
+                    gxi += cx; gyi += cy; gzi += cz;
+                    tLam += p.lt;
+                    tV += p.v;
+                }
+                // the lane that holds j = src gets this pair's terms: lane m receives from lane m - s
+                const int from = (lane - s) & 31;
+                sj += shfl_from(p.t, from);
+                if (kEnergy) {
+                    gxj -= shfl_from(cx, from);
+                    gyj -= shfl_from(cy, from);
+                    gzj -= shfl_from(cz, from);
+                }
+            }
+            if (vj) {
+                atomicAdd(&ag[3 * NP + jb + lane], sj);
+                if (kEnergy) {
+                    atomicAdd(&ag[jb + lane], gxj);
+                    atomicAdd(&ag[NP + jb + lane], gyj);
+                    atomicAdd(&ag[2 * NP + jb + lane], gzj);
+                }
+            }
+        }
+        if (vi) {
+            atomicAdd(&ag[3 * NP + i], si);
+            if (kEnergy) {
+                atomicAdd(&ag[i], gxi);
+                atomicAdd(&ag[NP + i], gyi);
+                atomicAdd(&ag[2 * NP + i], gzi);
+            }
+        }
+    }
+    __syncthreads();
+
+    double tG2 = 0.0;
+    for (int i = tid; i < N; i += T) {
+        sv.S[(size_t)w * ld + i] = ag[3 * NP + i];                    // R17: rebuild the running sum
+        if (kEnergy) {
+            const double a = ag[i], b = ag[NP + i], c = ag[2 * NP + i];
+            tG2 += a * a + b * b + c * c;
+        }
+    }
+    if (kEnergy) {
+        // each unordered pair was seen once: the Laplacian sum over i counts it twice
+        tLam *= 2.0;
+        tLam = warp_sum(tLam); tG2 = warp_sum(tG2); tV = warp_sum(tV);
+        if (lane == 0) { red[warp] = tLam; red[32 + warp] = tG2; red[64 + warp] = tV; }
+        __syncthreads();
+        if (warp == 0) {
+            double a = lane < nwarps ? red[lane] : 0.0;
+            double b = lane < nwarps ? red[32 + lane] : 0.0;
+            double c = lane < nwarps ? red[64 + lane] : 0.0;
+            a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+            if (lane == 0) {
+                const double Dku = Dk * g.inv_unit * g.inv_unit;
+                const double lam = -5.0 * g.b5 * a;                            // sum_i Lambda_i
+                const double g2 = (2.5 * g.b5) * (2.5 * g.b5) * b;             // sum_i |G_i|^2
+                const double T_PB = -Dku * (lam + g2);
+                const double T_JF = -0.5 * Dku * lam;
+                double *o = out + (size_t)w * 4;
+                o[0] = c + T_PB; o[1] = c; o[2] = T_PB; o[3] = T_JF;
+            }
+        }
+    }
+}
+
+int smem_bytes64(int N) { return 98 * 8 + 7 * (((N + 31) >> 5) << 5) * 8; }
+
+template <int T>
+cudaError_t launch64(qmc_ctx *c, double *d_out, bool energy)
+{
+    const int smem = smem_bytes64(c->p.N);
+    cudaError_t e;
+    if (energy) {
+        auto k = energy64_kernel<T, true>;
+        if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
+        k<<<c->W, T, smem, c->stream>>>(c->sv, c->p.hbar2_over_2m, d_out);
+    } else {
+        auto k = energy64_kernel<T, false>;
+        if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
+        k<<<c->W, T, smem, c->stream>>>(c->sv, c->p.hbar2_over_2m, d_out);
+    }
+    return cudaGetLastError();
+}
+
+template <int T>
+int occupancy64(int smem)
+{
+    int occ = 0;
+    auto k = energy64_kernel<T, true>;
+    cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, T, smem);
+    return occ;
+}
+
+}  // namespace
+
+#define QMC_E64_THREADS(X) X(32) X(64) X(128) X(256) X(512)
+
+cudaError_t launch_energy_f64(qmc_ctx *c, double *d_out, bool energy)
+{
+    const int T = c->energy_plan.threads;
+#define X(TT) if (T == TT) return launch64<TT>(c, d_out, energy);
+    QMC_E64_THREADS(X)
+#undef X
+    return cudaErrorInvalidValue;
+}
+
+// One warp per 64 particles (a block of 32 has about n/2 block pairs to go through), 1 to 8 warps;
+// QMC_ENERGY_THREADS overrides (tuning experiments).  false: N too large for the per-particle
+// accumulators in shared memory -- the caller falls back to the ordered-pair kernel of qmc_energy.cu.
+bool plan_energy_f64(qmc_ctx *c, EnergyPlan *out)
+{
+    const int N = c->p.N;
+    const int smem = smem_bytes64(N);
+    if (smem > 227 * 1024) return false;
+    int T = 32;
+    while (2 * T < N && T < 256) T *= 2;
+    if (const char *env = getenv("QMC_ENERGY_THREADS")) {
+        const int v = atoi(env);
+        if (v >= 32 && v <= 512 && (v & (v - 1)) == 0) T = v;
+    }
+    out->threads = T;
+    out->smem_bytes = smem;
+    out->variant = 1;
+    out->ctas_per_sm = 0;
+#define X(TT) if (T == TT) out->ctas_per_sm = occupancy64<TT>(smem);
+    QMC_E64_THREADS(X)
+#undef X
+    return true;
+}
+
+}  // namespace qmc

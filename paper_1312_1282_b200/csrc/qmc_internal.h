@@ -29,7 +29,7 @@ struct TraceView {
 };
 
 struct SweepPlan  { int threads, J, V, smem_bytes, ctas_per_sm; const void *shape; };
-struct EnergyPlan { int threads, smem_bytes, ctas_per_sm; };
+struct EnergyPlan { int threads, smem_bytes, ctas_per_sm, variant; };   // variant 1 (FP64): unordered-pair kernel
 
 }  // namespace qmc
 
@@ -71,5 +71,7 @@ bool plan_sweep(qmc_ctx *c, SweepPlan *out);
 bool plan_energy(qmc_ctx *c, EnergyPlan *out);
 cudaError_t launch_energy_f32(qmc_ctx *c, double *d_out, bool energy);
 bool plan_energy_f32(qmc_ctx *c, EnergyPlan *out);
+cudaError_t launch_energy_f64(qmc_ctx *c, double *d_out, bool energy);
+bool plan_energy_f64(qmc_ctx *c, EnergyPlan *out);
 
 }  // namespace qmc
