@@ -253,6 +253,9 @@ def main():
 
     # ---- roofline of the dominant kernel (the sweep): plain-ALU bound ---------------------------
     peak_meas = binding.pipe_peak(0 if w.mode == wl.MODE_FP64 else 1)
+    # live instruction rates of the other pipes the pair loop leans on (thread-level instr/s)
+    rates = {"ffma2": binding.pipe_peak(2), "mufu_rsq": binding.pipe_peak(3), "i2f": binding.pipe_peak(4),
+             "f2f": binding.pipe_peak(5)}
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     peak_derived = info["sm_count"] * LANES_PER_SM[w.mode] * sm_max * 1e6        # lane-instr/s
     t_launch = t_sweep / K
@@ -269,6 +272,12 @@ def main():
         "note": "achieved counts ONE trial evaluation per (moved, other) pair; executed_frac adds the "
                 "accepted-move re-evaluations the running-sum update performs (x(1+acceptance))",
         "kernel_ms": 1e3 * t_launch,
+        # the special-function unit (MUFU: 16 lanes per SM) is the co-limiter of the FP32C pair loop:
+        # 2 MUFU per u-evaluation (rsqrt, rcp); fp64 mode issues the same two (64H seeds)
+        "xu": {"peak_measured_G_instr_s": rates["mufu_rsq"] / 1e9,
+               "frac": sweep_pairs * 2.0 / t_launch / rates["mufu_rsq"],
+               "executed_frac": sweep_pairs * (1.0 + acc) * 2.0 / t_launch / rates["mufu_rsq"]},
+        "pipe_rates_measured_G_instr_s": {k: v / 1e9 for k, v in rates.items()},
     }
 
     out = {

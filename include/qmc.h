@@ -128,9 +128,10 @@ typedef struct {
 } qmc_info_t;
 int qmc_info(const qmc_ctx *c, qmc_info_t *out);
 
-/* FP pipe peak microbenchmark: runs a dependent-chain-free FMA kernel on
- * every SM and reports thread-level FMA instructions per second (host out, synchronous).
- * which: 0 = fp64 DFMA, 1 = fp32 FFMA. */
+/* Instruction-rate microbenchmark: runs a dependent-chain-free kernel of ONE
+ * instruction kind on every SM and reports thread-level instructions per second (host out, synchronous).
+ * which: 0 = fp64 DFMA, 1 = fp32 FFMA, 2 = packed FFMA2 (fma.rn.f32x2; two FMAs per instruction),
+ * 3 = MUFU.RSQ (fp32 rsqrt.approx), 4 = I2FP (s32 -> f32), 5 = F2F (f64 -> f32 -> f64, both counted). */
 int qmc_pipe_peak(int32_t which, void *cuda_stream, double *h_fma_per_s);
 
 #ifdef __cplusplus

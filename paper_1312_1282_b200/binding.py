@@ -105,7 +105,8 @@ def _make_params(N, walkers_per_group, box_L, jastrow_b, hbar2_over_2m, aziz, mo
 
 
 def pipe_peak(which: int, stream=None) -> float:
-    """Thread-level FMA instructions per second of the fp64 (0) or fp32 (1) pipe, measured live."""
+    """Thread-level instructions per second of one instruction kind, measured live (qmc.h: 0 DFMA,
+    1 FFMA, 2 FFMA2, 3 MUFU.RSQ, 4 I2FP, 5 F2F)."""
     import torch
     lib = load_library()
     st = torch.cuda.current_stream() if stream is None else stream
