@@ -21,9 +21,15 @@
 // exactly 0 -- one DSETP on the fp64 pipe, the selects run on the integer pipe.
 #include "qmc_internal.h"
 
+#ifndef QMC_E64_UNROLL
+#define QMC_E64_UNROLL 1
+#endif
+
 namespace qmc {
 
 namespace {
+
+constexpr int kUnroll64 = QMC_E64_UNROLL;            // pair steps in flight per lane
 
 struct Const64 {
     double L, h, h2, sh;
@@ -46,6 +52,28 @@ __device__ __forceinline__ double min_image(double a, double b, double h)
     const double m = h - fabs(f);
     const int hi = __double2hiint(m) | ((__double2hiint(d) ^ __double2hiint(f)) & 0x80000000);
     return __hiloint2double(hi, __double2loint(m));
+}
+
+// exp(a) for a <= 0 in fp64: a = n ln2 + r, |r| <= ln2/2, Taylor polynomial of degree 12 (remainder
+// < 2e-16 relative), 2^n through the exponent field; results below 2^-1022 come out as ~1e-308 instead
+// of a subnormal (they multiply a term that is then < 1e-300 K).  The coefficients sit in constant
+// memory so that every DFMA reads its coefficient as an operand (CUDA's exp() rebuilds its 64-bit
+// immediates with two uniform moves each inside the pair loop: 22 issue slots per pair).
+__constant__ double kExpC[13] = {
+    1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320, 1.0 / 362880,
+    1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600};
+__device__ __forceinline__ double exp_neg(double a)
+{
+    const double magic = 6755399441055744.0;                       // 2^52 + 2^51
+    const double t = fma(a, 1.4426950408889634, magic);
+    const double n = t - magic;
+    double r = fma(n, -6.93147180369123816490e-01, a);
+    r = fma(n, -1.90821492927058770002e-10, r);
+    double p = kExpC[12];
+#pragma unroll
+    for (int k = 11; k >= 0; --k) p = fma(p, r, kExpC[k]);
+    const int e = max(__double2loint(t), -1022);
+    return __hiloint2double(__double2hiint(p) + (e << 20), __double2loint(p));
 }
 
 struct Pair64 { double mx, my, mz, t, gm, lt, v; bool in; };
@@ -81,10 +109,10 @@ __device__ __forceinline__ Pair64 pair64(double xi, double yi, double zi, double
         double F = 1.0;
         if (__any_sync(0xffffffffu, x < C.D)) {
             const double q = fma(C.Drm, y, -1.0);                   // D/x - 1
-            const double e = exp(-q * q);
+            const double e = exp_neg(-q * q);
             F = x < C.D ? e : 1.0;
         }
-        const double rep = C.A * exp(x * fma(C.beta, x, -C.alpha));
+        const double rep = C.A * exp_neg(x * fma(C.beta, x, -C.alpha));
         p.v = p.in ? C.eps * fma(-F, disp, rep) : 0.0;
     }
     return p;
@@ -149,6 +177,7 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
             const bool vj = jb + lane < N;
             double gxj = 0.0, gyj = 0.0, gzj = 0.0, sj = 0.0;
             const int s0 = (k == 0) ? 1 : 0, s1 = (k == 0) ? 17 : 32;
+#pragma unroll kUnroll64
             for (int s = s0; s < s1; ++s) {
                 const int src = (lane + s) & 31;
                 const bool ok = vi && (jb + src < N) && !(k == 0 && s == 16 && lane >= 16);
