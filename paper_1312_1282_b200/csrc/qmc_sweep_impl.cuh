@@ -196,7 +196,7 @@ __device__ __forceinline__ double sum_parts(const double *pb)
 // <= 16 fp32 terms, are summed in fp32 before they reach the fp64 accumulator) -- this takes the
 // fp32 -> fp64 conversions, which run at 1/8 rate, off the per-pair path of an accepted move.
 constexpr int kFold = 16;
-template <typename Real, int T, int J, int V, int PD>
+template <typename Real, int T, int J, int V, int PD, bool DBG>
 __global__ void __launch_bounds__(T, (sweep_min_ctas<Real, T, J, PD>()))
 sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
 {
@@ -300,7 +300,7 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
         const Coord ty = trial_coord(ys, mr.dy);
         const Coord tz = trial_coord(zs, mr.dz);
         const double logxi = mr.logxi;
-        const bool owner = (tid == (s / V) % T);
+        const bool owner = ((unsigned)tid == (((unsigned)s / (unsigned)V) & (unsigned)(T - 1)));
         if (owner) x[s] = poison_of<Real>(tx);             // self term = 0 (nobody else reads x[s] during this move)
 
         // prefetch the next move: its particle cannot change in this move (N >= 3; else re-read below)
@@ -365,7 +365,7 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
         // a6: decision (Eq.(5), strict, log form: R8)
         const double margin = fma(c2, tot, -logxi);
         const bool accept = margin > 0.0;
-        if (tr.dec != nullptr) {
+        if (DBG && tr.dec != nullptr) {
             if (tid == 0 && w >= tr.w_begin && w < tr.w_end) {
                 const long long k = tr.offset + m;
                 if (k < tr.capacity) {
@@ -455,7 +455,7 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
         }
         s = sn;
         xs = xn; ys = yn; zs = zn;
-        if (N < 3) {                                        // degenerate: the next particle may just have moved
+        if (DBG && N < 3) {                                 // degenerate: the next particle may just have moved
             __syncthreads();
             xs = x[s]; ys = y[s]; zs = z[s];
             __syncthreads();
@@ -483,7 +483,9 @@ template <typename Real, int T, int J, int V, int PD>
 static cudaError_t shape_launch(qmc_ctx *c, int n_sweeps, int smem)
 {
     const uint2 key = make_uint2((uint32_t)(c->seed & 0xFFFFFFFFull), (uint32_t)(c->seed >> 32));
-    auto kern = sweep_kernel<Real, T, J, V, PD>;
+    // the lean instantiation has neither the decision trace nor the N < 3 re-read of the next particle
+    const bool dbg = c->trace.dec != nullptr || c->p.N < 3;
+    auto kern = dbg ? sweep_kernel<Real, T, J, V, PD, true> : sweep_kernel<Real, T, J, V, PD, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     kern<<<c->W, T, smem, c->stream>>>(c->sv, c->trace, key, c->t, n_sweeps);
@@ -494,7 +496,7 @@ template <typename Real, int T, int J, int V, int PD>
 static int shape_occupancy(int smem)
 {
     int n = 0;
-    auto kern = sweep_kernel<Real, T, J, V, PD>;
+    auto kern = sweep_kernel<Real, T, J, V, PD, false>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, T, smem) != cudaSuccess) return 0;
     return n;
