@@ -314,6 +314,42 @@ def test_fp32c_pair_sums_do_not_drift(qmc):
     assert not np.array_equal(S, S2)
 
 
+def test_fp32c_pending_sum_shape_matches_default(qmc, monkeypatch):
+    """The PD = 1 sweep shapes (S_j changes of <= 16 moves collected in fp32, R20) against the default
+    shape on the same walkers: running sums equal to fp32 accuracy, acceptance equal to a few flipped near-ties.
+    GPU-internal: the default shape is the one pinned to the oracle above."""
+    N, W = 256, 6
+    q0, L = make(qmc, N, W, qmc.QMC_FP32C)
+    monkeypatch.setenv("QMC_SWEEP_SHAPE", "64,8,4,1")
+    q1, _ = make(qmc, N, W, qmc.QMC_FP32C)
+    monkeypatch.delenv("QMC_SWEEP_SHAPE")
+    assert q1.info()["sweep_threads"] == 64 and q1.info()["sweep_pairs_per_thread"] == 8
+    for q in (q0, q1):
+        q.init_walkers(21)
+        q.sweep(3, 1.0)
+    S0, S1 = q0.pair_sums().cpu().numpy(), q1.pair_sums().cpu().numpy()
+    same = np.array([np.array_equal(a, b) for a, b in zip(q0.get_positions().cpu().numpy(), q1.get_positions().cpu().numpy())])
+    assert same.sum() >= W - 1                       # a near-tie may send one chain another way
+    assert np.abs(S0[same] - S1[same]).max() < 2e-5 * np.abs(S0).max()
+    q1.local_energy()                                 # rebuild: pending sums must have been folded in
+    S1r = q1.pair_sums().cpu().numpy()
+    assert np.abs(S1 - S1r).max() < 2e-5 * np.abs(S1r).max()
+
+
+def test_local_energy_fp64_ordered_fallback(qmc, oracle, monkeypatch):
+    """The ordered-pair fp64 energy kernel (used when the unordered-pair kernel's accumulators do not fit
+    shared memory) against the oracle."""
+    monkeypatch.setenv("QMC_ENERGY_ORDERED", "1")
+    N, W = 300, 3
+    q, L = make(qmc, N, W, qmc.QMC_FP64)
+    monkeypatch.delenv("QMC_ENERGY_ORDERED")
+    xyz = np.stack([wl.liquid_configuration(N, L, 900 + k) for k in range(W)])
+    q.set_positions(xyz)
+    eg = q.local_energy().cpu().numpy()
+    eo = oracle.local_energy(orc_sys(oracle, N, L), xyz)
+    assert relerr(eg, eo[:, :4]).max() < TOL64, (eg, eo)
+
+
 # ------------------------------------------------------------------------------ boundary behaviour
 def test_error_codes(qmc):
     with pytest.raises(qmc.QmcError) as e:
