@@ -151,7 +151,8 @@ static inline int sweep_smem_bytes(int T, int J, int mode, int P)
 {
     const int real = (mode == QMC_FP64) ? 8 : 4;
     const int NP = T * J;
-    return NP * 8 + 2 * kChunk * 32 + 64 * 8 + 3 * NP * real + (P ? NP * 4 : 0);
+    (void)P;                                             // hi + lo takes the room of the fp64 sums
+    return NP * 8 + 2 * kChunk * 32 + 64 * 8 + 3 * NP * real;
 }
 
 // Resident CTAs per SM the register allocator should leave room for: what shared memory allows for
@@ -160,7 +161,7 @@ template <typename Real, int T, int J, int P>
 constexpr int sweep_min_ctas()
 {
     const int real = (int)sizeof(Real);
-    const int smem = J * T * (8 + 3 * real + (P ? 4 : 0)) + 2 * kChunk * 32 + 64 * 8 + 1024;
+    const int smem = J * T * (8 + 3 * real) + 2 * kChunk * 32 + 64 * 8 + 1024;
     const int by_smem = (228 * 1024) / smem;
     const int regs = (real == 8 ? 96 + 3 * J : 40 + 3 * J);
     const int by_regs = 65536 / (regs * T);
@@ -191,10 +192,15 @@ __device__ __forceinline__ double sum_parts(const double *pb)
 
 // T threads per CTA; each thread owns J particles in G = J/V packs of V consecutive ones:
 // particle j = (g*T + tid)*V + e, g < G, e < V.  Shared arrays are padded to NP = T*J entries.
-// P = 1 (FP32C, V >= 2): the changes t_new - t_old of the running pair sums are first collected in an fp32
-// array `pend` and folded into the fp64 sums S every kFold moves (R20: at most kFold accepted moves, i.e.
-// <= 16 fp32 terms, are summed in fp32 before they reach the fp64 accumulator) -- this takes the
-// fp32 -> fp64 conversions, which run at 1/8 rate, off the per-pair path of an accepted move.
+// PD = 1 (FP32C, V >= 2): a running pair sum is held on chip as the unevaluated sum of two fp32 numbers
+// hi + lo (the same 8 bytes per particle as an fp64 sum).  An accepted move adds its fp32 changes
+// t_new - t_old to lo with packed adds; every kFold moves each thread renormalises its own sums with an
+// error-free TwoSum (hi + lo unchanged as a real number, |lo| <= ulp(hi)/2 again).  Between two
+// renormalisations lo has collected the changes of at most kFold moves in fp32 (R20: <= 16 fp32 terms are
+// summed in fp32 before they reach the wide accumulator); hi + lo carries 48 significant bits against the 24
+// of the pair terms that go into it.  This takes the fp32 -> fp64 conversions, which run at 1/8 rate on the
+// unit that also serves rsqrt and rcp, off the per-pair path of an accepted move; fp64 appears where a sum is
+// read (the owner of the moved particle) and when the state is stored.
 constexpr int kFold = 16;
 template <typename Real, int T, int J, int V, int PD, bool DBG>
 __global__ void __launch_bounds__(T, (sweep_min_ctas<Real, T, J, PD>()))
@@ -219,7 +225,7 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
     double         *part = reinterpret_cast<double *>(smem_raw + NP * 8 + 2 * kChunk * 32);   // [2][32]
     Coord          *x    = reinterpret_cast<Coord *>(part + 64);                              // [3][NP]
     Coord *y = x + NP, *z = x + 2 * NP;
-    float *pend = reinterpret_cast<float *>(x + 3 * NP);                                      // [NP] (P = 1 only)
+    float *Shi = reinterpret_cast<float *>(S), *Slo = Shi + NP;                               // PD = 1: S as hi + lo, [NP] each
     static_assert(sizeof(MoveRand<Real>) <= 32, "variate record must fit its 32-byte slot");
 
     const GroupDev g = sv.groups[sv.group_of[w]];
@@ -245,8 +251,13 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
             else                { cx = cy = cz = poison_of<Real>(Coord(0)); }
         }
         x[j] = cx; y[j] = cy; z[j] = cz;
-        S[s_index<T, V>(j)] = s;
-        if constexpr (kPend) pend[j] = 0.0f;
+        if constexpr (kPend) {
+            const float hi = __double2float_rn(s);
+            Shi[j] = hi;
+            Slo[j] = __double2float_rn(s - (double)hi);
+        } else {
+            S[s_index<T, V>(j)] = s;
+        }
     }
 
     // per-pack clamp bias of this thread (FP32C): 1 for padding packs.  Requires N % V == 0 (planner).
@@ -346,8 +357,9 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
         }
         double acc = (double)accr;
         if (owner) {                                       // a4: sum_j t_new - S_s
-            double Ss = S[s_index<T, V>(s)];
-            if constexpr (kPend) Ss += (double)pend[s];
+            double Ss;
+            if constexpr (kPend) Ss = (double)Shi[s] + (double)Slo[s];
+            else                 Ss = S[s_index<T, V>(s)];
             acc -= Ss;
         }
 
@@ -390,7 +402,7 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
                     S[base] += (double)(un[gi] - to);
                 } else if constexpr (kPend) {
                     using PackF = Pack<float, V>;
-                    PackF pd = *reinterpret_cast<const PackF *>(pend + base);
+                    PackF pd = *reinterpret_cast<const PackF *>(Slo + base);
 #pragma unroll
                     for (int c = 0; c < V / 2; ++c) {
                         const f32x2 to2 = pair_t2(xs, ys, zs, X.v[2 * c], X.v[2 * c + 1], Y.v[2 * c], Y.v[2 * c + 1],
@@ -398,7 +410,7 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
                         const f32x2 nw = add2(pk2(pd.v[2 * c], pd.v[2 * c + 1]), sub2(un2[(gi * V) / 2 + c], to2));
                         upk2(nw, pd.v[2 * c], pd.v[2 * c + 1]);
                     }
-                    *reinterpret_cast<PackF *>(pend + base) = pd;
+                    *reinterpret_cast<PackF *>(Slo + base) = pd;
                 } else {
 #pragma unroll
                     for (int c = 0; c < V / 2; ++c) {
@@ -422,8 +434,14 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
                 }
             }
             if (owner) {
-                if constexpr (kPend) { S[s_index<T, V>(s)] += (double)pend[s] + tot; pend[s] = 0.0f; }
-                else                 S[s_index<T, V>(s)] += tot;
+                if constexpr (kPend) {
+                    const double ns = (double)Shi[s] + (double)Slo[s] + tot;
+                    const float hi = __double2float_rn(ns);
+                    Shi[s] = hi;
+                    Slo[s] = __double2float_rn(ns - (double)hi);
+                } else {
+                    S[s_index<T, V>(s)] += tot;
+                }
                 x[s] = commit_coord(tx, g.L);
                 y[s] = commit_coord(ty, g.L);
                 z[s] = commit_coord(tz, g.L);
@@ -433,23 +451,24 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
             x[s] = xs;                                      // undo the poison
         }
         if constexpr (kPend) {
-            if ((m & (kFold - 1)) == kFold - 1 || m + 1 == total) {       // fold the pending changes into S
+            if ((m & (kFold - 1)) == kFold - 1) {             // renormalise this thread's sums: TwoSum(hi, lo)
 #pragma unroll
                 for (int gi = 0; gi < G; ++gi) {
                     using PackF = Pack<float, V>;
                     const int base = (gi * T + tid) * V;
-                    const PackF pd = *reinterpret_cast<const PackF *>(pend + base);
-                    PackF zr;
+                    PackF ph = *reinterpret_cast<const PackF *>(Shi + base);
+                    PackF pl = *reinterpret_cast<const PackF *>(Slo + base);
 #pragma unroll
                     for (int c = 0; c < V / 2; ++c) {
-                        double2 *sp = reinterpret_cast<double2 *>(S + ((gi * (V / 2) + c) * T + tid) * 2);
-                        double2 sv2 = *sp;
-                        sv2.x += (double)pd.v[2 * c];
-                        sv2.y += (double)pd.v[2 * c + 1];
-                        *sp = sv2;
-                        zr.v[2 * c] = 0.0f; zr.v[2 * c + 1] = 0.0f;
+                        const f32x2 h2 = pk2(ph.v[2 * c], ph.v[2 * c + 1]), l2 = pk2(pl.v[2 * c], pl.v[2 * c + 1]);
+                        const f32x2 sm = add2(h2, l2);
+                        const f32x2 bb = sub2(sm, h2);
+                        const f32x2 er = add2(sub2(h2, sub2(sm, bb)), sub2(l2, bb));
+                        upk2(sm, ph.v[2 * c], ph.v[2 * c + 1]);
+                        upk2(er, pl.v[2 * c], pl.v[2 * c + 1]);
                     }
-                    *reinterpret_cast<PackF *>(pend + base) = zr;
+                    *reinterpret_cast<PackF *>(Shi + base) = ph;
+                    *reinterpret_cast<PackF *>(Slo + base) = pl;
                 }
             }
         }
@@ -467,7 +486,8 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
     for (int j = tid; j < N; j += T) {
         if constexpr (kF32) { gpos[j] = dec_coord(x[j]); gpos[ld + j] = dec_coord(y[j]); gpos[2 * ld + j] = dec_coord(z[j]); }
         else                { gpos[j] = x[j]; gpos[ld + j] = y[j]; gpos[2 * ld + j] = z[j]; }
-        gS[j] = S[s_index<T, V>(j)];
+        if constexpr (kPend) gS[j] = (double)Shi[j] + (double)Slo[j];
+        else                 gS[j] = S[s_index<T, V>(j)];
     }
     if (tid == 0) sv.n_acc[w] += n_acc;
 }

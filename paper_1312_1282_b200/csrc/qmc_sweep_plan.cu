@@ -42,7 +42,7 @@ bool plan_sweep(qmc_ctx *c, SweepPlan *out)
             if (!usable(tab[k])) continue;
             const double waste = (double)(tab[k].T * tab[k].J - N) / (double)N;       // idle slots
             const double score = 4.0 * waste + std::fabs(std::log2((double)tab[k].T) - t_target)
-                               + (mode == QMC_FP64 ? 0.25 * (2 - tab[k].V) : 0.25 * (4 - tab[k].V)) + 0.1 * tab[k].P;   // pending sums cost a resident CTA at N = 1952 (measured: 11.8 vs 11.45 ms)
+                               + (mode == QMC_FP64 ? 0.25 * (2 - tab[k].V) : 0.25 * (4 - tab[k].V)) - 0.1 * tab[k].P;   // hi + lo running sums: 10.5 vs 11.1 ms at N = 1952 (measured)
             if (score < best_score) { best_score = score; best = &tab[k]; }
         }
     }

@@ -314,13 +314,13 @@ def test_fp32c_pair_sums_do_not_drift(qmc):
     assert not np.array_equal(S, S2)
 
 
-def test_fp32c_pending_sum_shape_matches_default(qmc, monkeypatch):
-    """The PD = 1 sweep shapes (S_j changes of <= 16 moves collected in fp32, R20) against the default
-    shape on the same walkers: running sums equal to fp32 accuracy, acceptance equal to a few flipped near-ties.
+def test_fp32c_sum_representations_agree(qmc, monkeypatch):
+    """A PD = 0 sweep shape (fp64 running sums in shared memory) against the default PD = 1 shape (sums held as
+    an fp32 pair hi + lo, R20) on the same walkers: running sums equal to fp32 accuracy, acceptance equal to a few flipped near-ties.
     GPU-internal: the default shape is the one pinned to the oracle above."""
     N, W = 256, 6
     q0, L = make(qmc, N, W, qmc.QMC_FP32C)
-    monkeypatch.setenv("QMC_SWEEP_SHAPE", "64,8,4,1")
+    monkeypatch.setenv("QMC_SWEEP_SHAPE", "64,8,4,0")
     q1, _ = make(qmc, N, W, qmc.QMC_FP32C)
     monkeypatch.delenv("QMC_SWEEP_SHAPE")
     assert q1.info()["sweep_threads"] == 64 and q1.info()["sweep_pairs_per_thread"] == 8
@@ -331,7 +331,7 @@ def test_fp32c_pending_sum_shape_matches_default(qmc, monkeypatch):
     same = np.array([np.array_equal(a, b) for a, b in zip(q0.get_positions().cpu().numpy(), q1.get_positions().cpu().numpy())])
     assert same.sum() >= W - 1                       # a near-tie may send one chain another way
     assert np.abs(S0[same] - S1[same]).max() < 2e-5 * np.abs(S0).max()
-    q1.local_energy()                                 # rebuild: pending sums must have been folded in
+    q1.local_energy()                                 # rebuild from scratch
     S1r = q1.pair_sums().cpu().numpy()
     assert np.abs(S1 - S1r).max() < 2e-5 * np.abs(S1r).max()
 
