@@ -144,6 +144,9 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--walkers", type=int, default=None, help="truncate walkers per group (debugging)")
+    ap.add_argument("--time-to-error", type=int, default=0, metavar="S",
+                    help="after the timed steps: S more steps with the energy recorded, reblocked -> the paper's "
+                         "t*sigma^2 and seconds to 1 mK per atom (PAPER.md l.504-511); 0 = skip")
     args = ap.parse_args()
 
     w = wl.config(args.config)
@@ -304,6 +307,36 @@ def main():
         "gpu_launches": int(launches),
         "roofline": roofline,
     }
+    # ---- observables beside the hot path: g(r) histogram, time to error ----
+    nb = 256
+    if 24 * N + 4 * nb <= 227 * 1024:
+        hist = torch.empty((W, nb), dtype=torch.int32, device=dev)
+        q.pair_histogram(nb, hist)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(3):
+            q.pair_histogram(nb, hist)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 3
+        out["observables"] = {"pair_histogram_ms": ms, "pairs_per_s": W * N * (N - 1) / 2 / (ms * 1e-3), "nbins": nb,
+                              "pairs_inside_cutoff_per_walker": float(hist.sum(1).double().mean())}
+    if args.time_to_error > 0:
+        from paper_1312_1282_b200 import observables as ob
+        S = args.time_to_error
+        series = []
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(S):
+            one_step()
+            series.append(e_out[:, 0].mean().item() / N)       # walker-averaged E_PB per atom of this step
+        el = time.perf_counter() - t0
+        mean, se, tau = ob.reblock(series, min_blocks=8)
+        tsig, t_goal = ob.seconds_to_error(se, el)
+        out["time_to_error"] = {"steps": S, "seconds": el, "E_per_atom_K": mean, "se_K": se, "tau_steps": tau,
+                                "t_sigma2_s_mK2": tsig, "seconds_to_1mK_per_atom": t_goal,
+                                "note": "chain continues from the timed steps (not equilibrated if few steps were run)"}
     if not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w, m)
     print(json.dumps(out))

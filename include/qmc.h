@@ -88,6 +88,13 @@ int qmc_sweep(qmc_ctx *c, int32_t n_sweeps, const double *steps);
  * Also rebuilds the running pair sums S_i from scratch (R17). */
 int qmc_local_energy(qmc_ctx *c, double *d_out);
 
+/* Pair-distance histogram of every walker's current configuration, the raw data of the pair distribution
+ * function g(r) (l.421, l.468): d_hist device [W][nbins] uint32, bin k counts the
+ * pairs i < j with minimum-image distance r in [k, k+1) * (L/2)/nbins; pairs with r >= L/2 are not counted.
+ * The bin of a pair is specified to the bit, so counts are reproducible exactly.
+ * 1 <= nbins <= 8192; QMC_E_CAPACITY if 24 N + 4 nbins bytes exceed one CTA's shared memory. */
+int qmc_pair_histogram(qmc_ctx *c, int32_t nbins, uint32_t *d_hist);
+
 /* d_out: device [W] accepted / attempted moves since qmc_init_walkers / qmc_set_positions. */
 int qmc_acceptance(qmc_ctx *c, double *d_out);
 

@@ -62,6 +62,7 @@ def _load():
                                            C.c_double, u8p, dp, u8p, C.POINTER(C.c_int64)]
         _lib.orc_local_energy_walkers.argtypes = [sp, dp, C.c_int32, dp]
         _lib.orc_num_threads.restype = C.c_int32
+        _lib.orc_pair_histogram.argtypes = [sp, dp, C.c_int, C.POINTER(C.c_uint32)]
     return _lib
 
 
@@ -187,4 +188,18 @@ def local_energy(sys: System, xyz) -> np.ndarray:
     assert x.shape[1:] == (3, sys.N)
     out = np.zeros((x.shape[0], 6))
     _load().orc_local_energy_walkers(sys.ref, _dp(x), x.shape[0], _dp(out))
+    return out
+
+
+def pair_histogram(sys: System, xyz, nbins: int) -> np.ndarray:
+    """[W][nbins] uint32: counts of pair distances r < L/2 in bins of width (L/2)/nbins, per configuration
+    (pair distribution function)."""
+    x = _f64(xyz)
+    if x.ndim == 2:
+        x = x[None]
+    assert x.shape[1:] == (3, sys.N)
+    out = np.zeros((x.shape[0], nbins), np.uint32)
+    for w in range(x.shape[0]):
+        xw = np.ascontiguousarray(x[w])
+        _load().orc_pair_histogram(sys.ref, _dp(xw), nbins, out[w].ctypes.data_as(C.POINTER(C.c_uint32)))
     return out

@@ -381,3 +381,31 @@ int32_t orc_num_threads(void)
 #endif
     return n;
 }
+
+/* ---------------------------------------------------------------------------
+ * Pair distribution function (the paper's second observable, l.421, l.468): histogram of the
+ * minimum-image pair distances of ONE configuration.  Bins of width h / nbins on [0, h), h = L/2
+ * (the cutoff of l.460).  For every pair i < j with r < h: k = (int)(r * inv_dr), inv_dr = nbins / h;
+ * k = nbins (r within rounding of h) is counted in the last bin.  DESIGN.md "Observables".
+ * ------------------------------------------------------------------------- */
+void orc_pair_histogram(const orc_sys *sys, const double *xyz, int nbins, uint32_t *hist)
+{
+    const int N = sys->N;
+    const double h = 0.5 * sys->L;
+    const double inv_dr = (double)nbins / h;
+    for (int k = 0; k < nbins; ++k) hist[k] = 0u;
+    for (int i = 0; i < N; ++i) {
+        double pi[3];
+        get_pos(xyz, N, i, pi);
+        for (int j = i + 1; j < N; ++j) {
+            double pj[3];
+            get_pos(xyz, N, j, pj);
+            const double r = dist(pi, pj, sys->L);
+            if (r < h) {
+                int k = (int)(r * inv_dr);
+                if (k >= nbins) k = nbins - 1;
+                hist[k] += 1u;
+            }
+        }
+    }
+}

@@ -21,7 +21,7 @@ EXPORTS = (
     "qmc_state_bytes", "qmc_create", "qmc_destroy", "qmc_init_walkers", "qmc_sweep", "qmc_local_energy",
     "qmc_acceptance", "qmc_step_host", "qmc_last_error", "qmc_get_positions", "qmc_set_positions",
     "qmc_set_seed", "qmc_get_pair_sums", "qmc_refresh_pair_sums", "qmc_trace_decisions", "qmc_info",
-    "qmc_pipe_peak",
+    "qmc_pipe_peak", "qmc_pair_histogram",
 )
 
 
@@ -77,6 +77,7 @@ def load_library() -> C.CDLL:
     lib.qmc_sweep.argtypes = [vp, C.c_int32, dp]
     lib.qmc_local_energy.argtypes = [vp, vp]
     lib.qmc_acceptance.argtypes = [vp, vp]
+    lib.qmc_pair_histogram.argtypes = [vp, C.c_int32, vp]
     lib.qmc_step_host.argtypes = [vp, vp, C.c_int32, dp, vp, vp, vp]
     lib.qmc_last_error.argtypes = [vp]
     lib.qmc_last_error.restype = C.c_char_p
@@ -212,6 +213,14 @@ class QMC:
         if out is None:
             out = torch.empty((self.W,), dtype=torch.float64, device=self.device)
         self._check(self._lib.qmc_acceptance(self._ctx, self._ptr(out, torch.float64, self.W)))
+        return out
+
+    def pair_histogram(self, nbins: int, out=None):
+        """[W][nbins] int32 tensor of pair-distance counts (uint32 on the C side; counts stay below 2^31)."""
+        torch = self._torch
+        if out is None:
+            out = torch.empty((self.W, nbins), dtype=torch.int32, device=self.device)
+        self._check(self._lib.qmc_pair_histogram(self._ctx, int(nbins), self._ptr(out, torch.int32, self.W * nbins)))
         return out
 
     def step_host(self, n_sweeps: int, steps, h_xyz_in=None, h_energy=None, h_acc=None, h_xyz_out=None):

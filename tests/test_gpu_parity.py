@@ -350,6 +350,26 @@ def test_local_energy_fp64_ordered_fallback(qmc, oracle, monkeypatch):
     assert relerr(eg, eo[:, :4]).max() < TOL64, (eg, eo)
 
 
+# ------------------------------------------------------------------------------ pair distribution function
+@pytest.mark.parametrize("mode_name,N,nb", [("fp64", 2, 7), ("fp64", 100, 64), ("fp64", 515, 200), ("fp32c", 256, 128),
+                                            ("fp64", 1952, 512), ("fp32c", 1952, 512)])
+def test_pair_histogram_bit_exact(qmc, oracle, mode_name, N, nb):
+    """qmc_pair_histogram (NEXT-2) against the oracle on the configuration the GPU holds after a
+    few sweeps: integer counts, bit-exact (the bin arithmetic is specified to the bit)."""
+    mode = qmc.QMC_FP64 if mode_name == "fp64" else qmc.QMC_FP32C
+    W = 3
+    q, L = make(qmc, N, W, mode)
+    q.init_walkers(31)
+    q.sweep(2, 1.0 if N > 2 else 0.4)
+    Hg = q.pair_histogram(nb).cpu().numpy()
+    xyz = q.get_positions().cpu().numpy()
+    Ho = oracle.pair_histogram(orc_sys(oracle, N, L), xyz, nb)
+    assert np.array_equal(Hg.astype(np.int64), Ho.astype(np.int64))
+    assert Hg.sum() > 0 or N == 2
+    with pytest.raises(qmc.QmcError):
+        q.pair_histogram(0)
+
+
 # ------------------------------------------------------------------------------ boundary behaviour
 def test_error_codes(qmc):
     with pytest.raises(qmc.QmcError) as e:

@@ -413,3 +413,79 @@ def test_p6_paper_sample_run_energies(oracle):
     assert abs(T_jf - T_p) < 0.20, (T_jf, T_p)
     assert abs(T_pb - T_p) < 0.35, (T_pb, T_p)
     assert abs((V + T_jf) - E_p) < 0.20, (V + T_jf, E_p)
+
+
+# ------------------------------------------------------------------ pair distribution function (NEXT-2)
+def test_pair_histogram_against_brute_force_images(oracle):
+    """orc_pair_histogram against a numpy count over all 27 periodic images (nearest one wins)."""
+    N, nb = 40, 25
+    s = make_sys(oracle, N)
+    rng = np.random.default_rng(5)
+    xyz = rng.uniform(0.0, s.L, (3, N))
+    H = oracle.pair_histogram(s, xyz, nb)[0]
+    h = 0.5 * s.L
+    ref = np.zeros(nb, np.int64)
+    shifts = np.array([(a, b, c) for a in (-1, 0, 1) for b in (-1, 0, 1) for c in (-1, 0, 1)], float) * s.L
+    for i in range(N):
+        for j in range(i + 1, N):
+            d = xyz[:, i] - xyz[:, j]
+            r = np.sqrt(((d[None, :] + shifts) ** 2).sum(1)).min()
+            if r < h:
+                ref[min(int(r * nb / h), nb - 1)] += 1
+    assert np.array_equal(H, ref)
+    assert H.sum() == ref.sum() > 0
+
+
+def test_pair_histogram_fcc_shells(oracle):
+    """A perfect FCC lattice (N = 4 k^3, no jitter): 12 nearest neighbours at a/sqrt(2) -> 6N pairs, 6 second
+    neighbours at a -> 3N pairs, nothing below the first shell."""
+    N = 108                                            # k = 3
+    s = make_sys(oracle, N)
+    xyz = oracle.init_walkers(s, 1, 0, 1, 0.0)
+    a = s.L / 3.0
+    nb = 300
+    H = oracle.pair_histogram(s, xyz, nb)[0].astype(np.int64)
+    dr = 0.5 * s.L / nb
+    k1, k2 = int(a / math.sqrt(2.0) / dr), int(a / dr)
+    assert H[:k1 - 1].sum() == 0
+    assert H[k1 - 1:k1 + 2].sum() == 6 * N
+    assert H[k2 - 1:k2 + 2].sum() == 3 * N
+
+
+def test_g_of_r_of_an_ideal_gas_is_one(oracle):
+    """Normalisation of observables.g_of_r: uniform random points have g(r) = 1 within counting noise."""
+    from paper_1312_1282_b200 import observables as ob
+    N, W, nb = 400, 24, 20
+    s = make_sys(oracle, N)
+    rng = np.random.default_rng(11)
+    xyz = rng.uniform(0.0, s.L, (W, 3, N))
+    r, g = ob.g_of_r(oracle.pair_histogram(s, xyz, nb), N, s.L)
+    assert r.shape == g.shape == (nb,)
+    counts = oracle.pair_histogram(s, xyz, nb).sum(0)
+    sel = counts > 2000
+    assert sel.sum() >= 10
+    assert np.all(np.abs(g[sel] - 1.0) < 5.0 / np.sqrt(counts[sel]) + 2.0 / N)
+
+
+def test_reblock_recovers_the_error_of_an_ar1_series():
+    """observables.reblock on an AR(1) series with known integrated autocorrelation time
+    tau = (1 + phi) / (2 (1 - phi)): the blocked error must be ~sqrt(2 tau) times the naive one."""
+    from paper_1312_1282_b200 import observables as ob
+    rng = np.random.default_rng(3)
+    phi, n = 0.8, 1 << 16
+    e = rng.standard_normal(n)
+    x = np.empty(n)
+    x[0] = e[0]
+    for k in range(1, n):
+        x[k] = phi * x[k - 1] + e[k]
+    mean, se, tau = ob.reblock(x)
+    tau_exact = (1 + phi) / (2 * (1 - phi))
+    sigma2 = 1.0 / (1 - phi * phi)
+    se_exact = math.sqrt(2 * tau_exact * sigma2 / n)
+    assert abs(se / se_exact - 1.0) < 0.25
+    assert abs(tau / tau_exact - 1.0) < 0.5
+    assert abs(mean) < 5 * se_exact
+    m2, se2, tau2 = ob.reblock(rng.standard_normal(4096))
+    assert 0.8 < se2 * math.sqrt(4096) < 1.35 and tau2 < 1.0
+    tsig, t_goal = ob.seconds_to_error(2e-3, 10.0)
+    assert abs(tsig - 40.0) < 1e-9 and abs(t_goal - 40.0) < 1e-9
