@@ -144,6 +144,10 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--walkers", type=int, default=None, help="truncate walkers per group (debugging)")
+    ap.add_argument("--proposal", type=int, choices=[0, 1], default=0,
+                    help="0: particles in order, uniform cube (BASELINE.json); 1: the paper's random particle + "
+                         "Gaussian displacement (NEXT-1), standard deviation --sigma per component")
+    ap.add_argument("--sigma", type=float, default=0.8, help="proposal 1: standard deviation per component, Angstrom")
     ap.add_argument("--time-to-error", type=int, default=0, metavar="S",
                     help="after the timed steps: S more steps with the energy recorded, reblocked -> the paper's "
                          "t*sigma^2 and seconds to 1 mK per atom (PAPER.md l.504-511); 0 = skip")
@@ -180,6 +184,9 @@ def main():
                     walker_id_base=rank * W, jitter=wl.JITTER, device=str(dev))
     q.init_walkers(w.seed)
     steps = w.steps
+    if args.proposal == 1:
+        q.set_proposal(1)
+        steps = [args.sigma] * len(w.groups)
     e_out = torch.empty((W, 4), dtype=torch.float64, device=dev)
     a_out = torch.empty((W,), dtype=torch.float64, device=dev)
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)   # 256 MiB > 126 MB L2
@@ -290,6 +297,7 @@ def main():
         "dtype": "f32" if w.mode == wl.MODE_FP32C else "f64", "data": "synthetic",
         "config": {"workload": w.name, "N": N, "walkers_per_gpu": W, "groups": len(w.groups),
                    "sweeps_per_step": m, "mode": mode_name, "energy_every_step": True,
+                   "proposal": "ordered/uniform-cube" if args.proposal == 0 else f"random-particle/gaussian sigma={args.sigma} A",
                    "l2": "flushed between timed steps (256 MiB write, untimed)",
                    "sweep_threads": info["sweep_threads"], "sweep_ctas_per_sm": info["sweep_ctas_per_sm"],
                    "energy_threads": info["energy_threads"], "energy_ctas_per_sm": info["energy_ctas_per_sm"]},

@@ -83,6 +83,15 @@ int qmc_init_walkers(qmc_ctx *c, uint64_t seed);
  * sweep(a); sweep(b) == sweep(a+b). */
 int qmc_sweep(qmc_ctx *c, int32_t n_sweeps, const double *steps);
 
+/* Proposal of the following qmc_sweep calls.  kind 0 (default): particles in order,
+ * displacement uniform in [-step,step]^3 (BASELINE.json's reading, R7).  kind 1: the paper's own
+ * (l.144, l.325, l.347-349): each of the N moves of a sweep picks a random particle,
+ * s = floor(A0 N / 2^32), and displaces it by step * (z0, z1, z2), z standard normal by Box-Muller from
+ * Philox4x32-10 words A = (m,t,walker,2), B = (m,t,walker,3) (m = move index within the sweep); step is then the
+ * standard deviation per component and must satisfy 6.77 step < L/2.  The variate map is specified to the bit
+ * (DESIGN.md "Proposal 1"), so fp64 trajectories still match the oracle move for move. */
+int qmc_set_proposal(qmc_ctx *c, int32_t kind);
+
 /* Local energy of every walker's current configuration (l.113-115, l.129, l.381):
  * d_out: device [W][4] = E_PB, V, T_PB, T_JF, totals in K (divide by N for per-atom).
  * Also rebuilds the running pair sums S_i from scratch (R17). */

@@ -29,7 +29,7 @@ def build(force: bool = False) -> str:
 
 class _Sys(C.Structure):
     _fields_ = [("N", C.c_int32), ("L", C.c_double), ("b", C.c_double), ("Dk", C.c_double),
-                ("aziz", C.c_double * 9)]
+                ("aziz", C.c_double * 9), ("proposal", C.c_int32)]
 
 
 _lib = None
@@ -62,6 +62,9 @@ def _load():
                                            C.c_double, u8p, dp, u8p, C.POINTER(C.c_int64)]
         _lib.orc_local_energy_walkers.argtypes = [sp, dp, C.c_int32, dp]
         _lib.orc_num_threads.restype = C.c_int32
+        _lib.orc_normal_pair.argtypes = [C.c_uint32, C.c_uint32, dp]
+        _lib.orc_move_variates_gauss.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_int32, C.c_double,
+                                                 C.POINTER(C.c_int32), dp, dp]
         _lib.orc_pair_histogram.argtypes = [sp, dp, C.c_int, C.POINTER(C.c_uint32)]
     return _lib
 
@@ -77,9 +80,12 @@ def _f64(a) -> np.ndarray:
 class System:
     """N atoms in a cubic periodic box of edge L, Jastrow b, hbar^2/2m = Dk, potential constants."""
 
-    def __init__(self, N: int, L: float, b: float, Dk: float, aziz: Sequence[float]):
+    def __init__(self, N: int, L: float, b: float, Dk: float, aziz: Sequence[float], proposal: int = 0):
+        """proposal 0: particles in order, uniform cube (R7); 1: the paper's random particle +
+        Gaussian displacement of standard deviation `step` per component (l.144, l.325)."""
         self.N, self.L, self.b, self.Dk, self.aziz = int(N), float(L), float(b), float(Dk), tuple(aziz)
-        self._s = _Sys(self.N, self.L, self.b, self.Dk, (C.c_double * 9)(*self.aziz))
+        self.proposal = int(proposal)
+        self._s = _Sys(self.N, self.L, self.b, self.Dk, (C.c_double * 9)(*self.aziz), self.proposal)
 
     @property
     def ref(self):
@@ -203,3 +209,19 @@ def pair_histogram(sys: System, xyz, nbins: int) -> np.ndarray:
         xw = np.ascontiguousarray(x[w])
         _load().orc_pair_histogram(sys.ref, _dp(xw), nbins, out[w].ctypes.data_as(C.POINTER(C.c_uint32)))
     return out
+
+
+def normal_pair(w1: int, w2: int):
+    """Two standard normals from two 32-bit words (proposal 1's Box-Muller, bit-specified)."""
+    z = np.zeros(2)
+    _load().orc_normal_pair(w1, w2, _dp(z))
+    return float(z[0]), float(z[1])
+
+
+def move_variates_gauss(seed: int, w: int, t: int, m: int, N: int, step: float):
+    """(particle s, delta[3], xi) of move m of sweep t of walker w under proposal 1."""
+    d = np.zeros(3)
+    xi = C.c_double()
+    s = C.c_int32()
+    _load().orc_move_variates_gauss(seed, w, t, m, N, step, C.byref(s), _dp(d), C.byref(xi))
+    return int(s.value), d, float(xi.value)

@@ -27,6 +27,8 @@ typedef struct {
     double  b;        /* Jastrow parameter of Eq.(9), l.155                 */
     double  Dk;       /* hbar^2/2m, K*A^2                                   */
     double  aziz[9];  /* eps, rm, A, alpha, beta, c6, c8, c10, D  (R3)      */
+    int32_t proposal; /* 0: particles in order, uniform cube (R7); 1: the paper's random particle +
+                         Gaussian displacement (l.144, l.325)               */
 } orc_sys;
 
 /* ---------------------------------------------------------------------------
@@ -70,6 +72,93 @@ void orc_move_variates(uint64_t seed, uint32_t w, uint32_t t, uint32_t s, double
     orc_philox4x32_10(ctr, key, x);
     for (int k = 0; k < 3; ++k) delta[k] = step * unit_pm1(x[k]);
     *xi = unit_01(x[3]);
+}
+
+/* ---------------------------------------------------------------------------
+ * Proposal 1 (the paper's own, l.144 "a randomly selected particle", l.325 "Gaussian displacements" made
+ * by a Box-Muller kernel, l.347-349): written so that both implementations can reproduce every bit with
+ * IEEE +, -, *, /, sqrt alone; no library log / sin / cos.
+ *
+ *   ln u for u = (2 w + 1) 2^-33, w a 32-bit word: n = 2w + 1 = m 2^e, m in [1,2); m > sqrt2 -> m/2, e+1;
+ *   s = (m-1)/(m+1), ln m = 2 s P(s^2), P = sum_{k=0..10} s^2k/(2k+1) by Horner; ln u = ln m + (e-33) ln2.
+ *   cos, sin of 2 pi v for v = (w + 0.5) 2^-32: quadrant q = w >> 30, f = ((w & (2^30-1)) + 0.5) 2^-30;
+ *   f > 1/2: swap sin and cos of g = 1 - f; x = g pi/2 in (0, pi/4]; Taylor to x^15 / x^16 by Horner in x^2.
+ * ------------------------------------------------------------------------- */
+static double orc_ln_unit(uint32_t w)
+{
+    uint64_t n = 2ull * (uint64_t)w + 1ull;
+    int e = 0;
+    while ((n >> (e + 1)) != 0ull) ++e;                   /* e = floor(log2 n) */
+    double m = (double)n / (double)(1ull << e);           /* exact: n < 2^33 */
+    if (m > 1.4142135623730951) { m = 0.5 * m; e += 1; }
+    const double s = (m - 1.0) / (m + 1.0);
+    const double s2 = s * s;
+    double P = 1.0 / 21.0;
+    for (int k = 9; k >= 0; --k) P = P * s2 + 1.0 / (double)(2 * k + 1);
+    const double lnm = (2.0 * s) * P;
+    return lnm + (double)(e - 33) * 0.6931471805599453;
+}
+static void orc_cos_sin_2pi(uint32_t w, double *c, double *s)
+{
+    const uint32_t q = w >> 30;
+    double f = ((double)(w & 0x3FFFFFFFu) + 0.5) * (1.0 / 1073741824.0);
+    const int swap = f > 0.5;
+    if (swap) f = 1.0 - f;
+    const double x = f * 1.5707963267948966;
+    const double x2 = x * x;
+    double ps = -1.0 / 1307674368000.0;                   /* -1/15! */
+    ps = ps * x2 + 1.0 / 6227020800.0;                    /*  1/13! */
+    ps = ps * x2 - 1.0 / 39916800.0;
+    ps = ps * x2 + 1.0 / 362880.0;
+    ps = ps * x2 - 1.0 / 5040.0;
+    ps = ps * x2 + 1.0 / 120.0;
+    ps = ps * x2 - 1.0 / 6.0;
+    ps = ps * x2 + 1.0;
+    const double sn = x * ps;
+    double pc = 1.0 / 20922789888000.0;                   /*  1/16! */
+    pc = pc * x2 - 1.0 / 87178291200.0;                   /* -1/14! */
+    pc = pc * x2 + 1.0 / 479001600.0;
+    pc = pc * x2 - 1.0 / 3628800.0;
+    pc = pc * x2 + 1.0 / 40320.0;
+    pc = pc * x2 - 1.0 / 720.0;
+    pc = pc * x2 + 1.0 / 24.0;
+    pc = pc * x2 - 0.5;
+    pc = pc * x2 + 1.0;
+    const double c1 = swap ? sn : pc, s1 = swap ? pc : sn;   /* cos, sin of f pi/2 */
+    switch (q) {
+    case 0:  *c = c1;  *s = s1;  break;
+    case 1:  *c = -s1; *s = c1;  break;
+    case 2:  *c = -c1; *s = -s1; break;
+    default: *c = s1;  *s = -c1; break;
+    }
+}
+/* Box-Muller: two standard normals from two words. */
+void orc_normal_pair(uint32_t w1, uint32_t w2, double z[2])
+{
+    const double R = sqrt(-2.0 * orc_ln_unit(w1));
+    double c, s;
+    orc_cos_sin_2pi(w2, &c, &s);
+    z[0] = R * c;
+    z[1] = R * s;
+}
+/* Variates of move m of sweep t of walker w under proposal 1: words A = Philox(m,t,w,2), B = Philox(m,t,w,3);
+ * particle s = floor(A0 N / 2^32); (z0,z1) = BoxMuller(A1, A2), z2 = first of BoxMuller(B0, B1);
+ * delta[k] = step * z_k (ONE rounding); xi from A3 as in proposal 0. */
+void orc_move_variates_gauss(uint64_t seed, uint32_t w, uint32_t t, uint32_t m, int32_t N, double step,
+                             int32_t *s, double delta[3], double *xi)
+{
+    uint32_t key[2] = { (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32) };
+    uint32_t ca[4] = { m, t, w, 2u }, cb[4] = { m, t, w, 3u }, A[4], B[4];
+    orc_philox4x32_10(ca, key, A);
+    orc_philox4x32_10(cb, key, B);
+    *s = (int32_t)(((uint64_t)A[0] * (uint64_t)(uint32_t)N) >> 32);
+    double z01[2], z23[2];
+    orc_normal_pair(A[1], A[2], z01);
+    orc_normal_pair(B[0], B[1], z23);
+    delta[0] = step * z01[0];
+    delta[1] = step * z01[1];
+    delta[2] = step * z23[0];
+    *xi = unit_01(A[3]);
 }
 
 /* ---------------------------------------------------------------------------
@@ -200,7 +289,9 @@ static double wrap(double x, double L)
 
 /* ---------------------------------------------------------------------------
  * Metropolis sweeps of one walker (Eq.(5) l.123, Eq.(7) l.146, l.325-331; R7, R8).
- * For sweep t = t0 .. t0+n_sweeps-1, for s = 0 .. N-1 in order:
+ * For sweep t = t0 .. t0+n_sweeps-1, for s = 0 .. N-1 in order (proposal 1: N moves of the particle and
+ * Gaussian displacement orc_move_variates_gauss draws; |z| <= sqrt(66 ln 2) = 6.77 with 32-bit uniforms, and
+ * callers keep 6.77 step < L/2, so one wrap still brings a coordinate back into [0, L]):
  *   trial = r_s + delta;  accept iff 2*Delta > log(xi) (strict);
  *   on accept r_s <- wrap(trial).
  * Optional per-move outputs (index m = (t-t0)*N + s):
@@ -219,9 +310,11 @@ int64_t orc_sweep(const orc_sys *sys, double *xyz, uint64_t seed, uint32_t w, ui
     int64_t n_acc = 0, m = 0;
     for (int32_t it = 0; it < n_sweeps; ++it) {
         uint32_t t = t0 + (uint32_t)it;
-        for (int s = 0; s < N; ++s, ++m) {
+        for (int sq = 0; sq < N; ++sq, ++m) {
             double delta[3], xi, ps[3], trial[3];
-            orc_move_variates(seed, w, t, (uint32_t)s, step, delta, &xi);
+            int32_t s = sq;
+            if (sys->proposal == 1) orc_move_variates_gauss(seed, w, t, (uint32_t)sq, N, step, &s, delta, &xi);
+            else                    orc_move_variates(seed, w, t, (uint32_t)sq, step, delta, &xi);
             get_pos(xyz, N, s, ps);
             for (int k = 0; k < 3; ++k) trial[k] = ps[k] + delta[k];
             double Delta = orc_delta_log_psi(sys, xyz, s, trial);

@@ -21,7 +21,7 @@ EXPORTS = (
     "qmc_state_bytes", "qmc_create", "qmc_destroy", "qmc_init_walkers", "qmc_sweep", "qmc_local_energy",
     "qmc_acceptance", "qmc_step_host", "qmc_last_error", "qmc_get_positions", "qmc_set_positions",
     "qmc_set_seed", "qmc_get_pair_sums", "qmc_refresh_pair_sums", "qmc_trace_decisions", "qmc_info",
-    "qmc_pipe_peak", "qmc_pair_histogram",
+    "qmc_pipe_peak", "qmc_pair_histogram", "qmc_set_proposal",
 )
 
 
@@ -78,6 +78,7 @@ def load_library() -> C.CDLL:
     lib.qmc_local_energy.argtypes = [vp, vp]
     lib.qmc_acceptance.argtypes = [vp, vp]
     lib.qmc_pair_histogram.argtypes = [vp, C.c_int32, vp]
+    lib.qmc_set_proposal.argtypes = [vp, C.c_int32]
     lib.qmc_step_host.argtypes = [vp, vp, C.c_int32, dp, vp, vp, vp]
     lib.qmc_last_error.argtypes = [vp]
     lib.qmc_last_error.restype = C.c_char_p
@@ -214,6 +215,10 @@ class QMC:
             out = torch.empty((self.W,), dtype=torch.float64, device=self.device)
         self._check(self._lib.qmc_acceptance(self._ctx, self._ptr(out, torch.float64, self.W)))
         return out
+
+    def set_proposal(self, kind: int):
+        """0: particles in order, uniform cube; 1: random particle, Gaussian displacement (qmc.h)."""
+        self._check(self._lib.qmc_set_proposal(self._ctx, int(kind)))
 
     def pair_histogram(self, nbins: int, out=None):
         """[W][nbins] int32 tensor of pair-distance counts (uint32 on the C side; counts stay below 2^31)."""

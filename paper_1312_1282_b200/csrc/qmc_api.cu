@@ -325,6 +325,7 @@ extern "C" int qmc_create(const qmc_params *p, void *cuda_stream, void *d_state,
     c->sv.groups = c->d_groups;
     c->sv.W = c->W; c->sv.N = p->N; c->sv.ld = c->ld;
     c->sv.walker_id_base = p->walker_id_base;
+    c->sv.proposal = 0;
 
     if (!plan_sweep(c, &c->sweep_plan))
         CREATE_FAIL(QMC_E_CAPACITY, "N = %d does not fit the sweep kernel's shared-memory budget in mode %d "
@@ -378,6 +379,14 @@ extern "C" int qmc_set_seed(qmc_ctx *c, uint64_t seed, uint32_t t)
     return QMC_OK;
 }
 
+extern "C" int qmc_set_proposal(qmc_ctx *c, int32_t kind)
+{
+    if (!c) return QMC_E_ARG;
+    if (kind != 0 && kind != 1) QMC_FAIL(c, QMC_E_ARG, "unknown proposal kind %d", kind);
+    c->sv.proposal = kind;
+    return QMC_OK;
+}
+
 extern "C" int qmc_sweep(qmc_ctx *c, int32_t n_sweeps, const double *steps)
 {
     if (!c) return QMC_E_ARG;
@@ -387,8 +396,11 @@ extern "C" int qmc_sweep(qmc_ctx *c, int32_t n_sweeps, const double *steps)
     if ((long long)n_sweeps * c->p.N >= (1LL << 31)) QMC_FAIL(c, QMC_E_ARG, "n_sweeps * N must stay below 2^31 per call");
     bool changed = false;
     for (int g = 0; g < c->p.n_groups; ++g) {
-        if (!(steps[g] > 0.0) || !(steps[g] < 0.5 * c->box_L[g]))
-            QMC_FAIL(c, QMC_E_ARG, "steps[%d] = %g must lie in (0, L/2 = %g)", g, steps[g], 0.5 * c->box_L[g]);
+        // proposal 1: |z| <= sqrt(66 ln 2) < 6.77 with 32-bit uniforms; the displacement must stay below L/2
+        const double reach = c->sv.proposal == 1 ? 6.77 : 1.0;
+        if (!(steps[g] > 0.0) || !(steps[g] * reach < 0.5 * c->box_L[g]))
+            QMC_FAIL(c, QMC_E_ARG, "steps[%d] = %g must lie in (0, L/2 = %g)%s", g, steps[g], 0.5 * c->box_L[g],
+                     c->sv.proposal == 1 ? " after multiplication by 6.77 (largest Gaussian variate)" : "");
         if (c->groups[g].step != steps[g]) { c->groups[g].step = steps[g]; changed = true; }
     }
     if (changed)   // stream-ordered update of the small constant table (host mirror is ours, pageable copy is synchronous to the host)

@@ -67,6 +67,68 @@ __device__ __forceinline__ double word_to_unit(uint32_t x)
 }
 
 // ---------------------------------------------------------------------------------------------
+// Proposal 1 (PAPER.md l.144 random particle, l.325 Gaussian displacement by Box-Muller): standard normals
+// from 32-bit words with IEEE +, -, *, /, sqrt only, every operation rounded once in the order DESIGN.md
+// "Proposal 1" fixes, so that the CPU oracle's independent implementation agrees bit for bit.
+//   ln u, u = (2w+1) 2^-33:  n = 2w+1 = m 2^e, m in [1,2); m > sqrt2 -> m/2, e+1; s = (m-1)/(m+1);
+//                            ln m = 2 s sum_{k<=10} s^2k/(2k+1) (Horner), ln u = ln m + (e-33) ln2
+//   cos/sin 2 pi (w+1/2) 2^-32: quadrant w>>30, f from the low 30 bits; f > 1/2: use 1-f and swap;
+//                            x = f pi/2, Taylor in x^2 to x^15 (sin) and x^16 (cos) by Horner
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double ln_unit33(uint32_t w)
+{
+    const unsigned long long n = 2ull * (unsigned long long)w + 1ull;
+    int e = 63 - __clzll((long long)n);
+    double m = __ddiv_rn(__ull2double_rn(n), __ull2double_rn(1ull << e));
+    if (m > 1.4142135623730951) { m = __dmul_rn(0.5, m); e += 1; }
+    const double s = __ddiv_rn(__dadd_rn(m, -1.0), __dadd_rn(m, 1.0));
+    const double s2 = __dmul_rn(s, s);
+    double P = 1.0 / 21.0;
+#pragma unroll
+    for (int k = 9; k >= 0; --k) P = __dadd_rn(__dmul_rn(P, s2), 1.0 / (double)(2 * k + 1));
+    const double lnm = __dmul_rn(__dmul_rn(2.0, s), P);
+    return __dadd_rn(lnm, __dmul_rn((double)(e - 33), 0.6931471805599453));
+}
+__device__ __forceinline__ void cos_sin_2pi32(uint32_t w, double &c, double &s)
+{
+    const uint32_t q = w >> 30;
+    double f = __dmul_rn(__dadd_rn(__uint2double_rn(w & 0x3FFFFFFFu), 0.5), 1.0 / 1073741824.0);
+    const bool swap = f > 0.5;
+    if (swap) f = __dadd_rn(1.0, -f);
+    const double x = __dmul_rn(f, 1.5707963267948966);
+    const double x2 = __dmul_rn(x, x);
+    double ps = -1.0 / 1307674368000.0;
+    ps = __dadd_rn(__dmul_rn(ps, x2), 1.0 / 6227020800.0);
+    ps = __dadd_rn(__dmul_rn(ps, x2), -1.0 / 39916800.0);
+    ps = __dadd_rn(__dmul_rn(ps, x2), 1.0 / 362880.0);
+    ps = __dadd_rn(__dmul_rn(ps, x2), -1.0 / 5040.0);
+    ps = __dadd_rn(__dmul_rn(ps, x2), 1.0 / 120.0);
+    ps = __dadd_rn(__dmul_rn(ps, x2), -1.0 / 6.0);
+    ps = __dadd_rn(__dmul_rn(ps, x2), 1.0);
+    const double sn = __dmul_rn(x, ps);
+    double pc = 1.0 / 20922789888000.0;
+    pc = __dadd_rn(__dmul_rn(pc, x2), -1.0 / 87178291200.0);
+    pc = __dadd_rn(__dmul_rn(pc, x2), 1.0 / 479001600.0);
+    pc = __dadd_rn(__dmul_rn(pc, x2), -1.0 / 3628800.0);
+    pc = __dadd_rn(__dmul_rn(pc, x2), 1.0 / 40320.0);
+    pc = __dadd_rn(__dmul_rn(pc, x2), -1.0 / 720.0);
+    pc = __dadd_rn(__dmul_rn(pc, x2), 1.0 / 24.0);
+    pc = __dadd_rn(__dmul_rn(pc, x2), -0.5);
+    pc = __dadd_rn(__dmul_rn(pc, x2), 1.0);
+    const double c1 = swap ? sn : pc, s1 = swap ? pc : sn;
+    c = (q == 0) ? c1 : (q == 1) ? -s1 : (q == 2) ? -c1 : s1;
+    s = (q == 0) ? s1 : (q == 1) ? c1 : (q == 2) ? -s1 : -c1;
+}
+__device__ __forceinline__ void normal_pair(uint32_t w1, uint32_t w2, double &z0, double &z1)
+{
+    const double R = __dsqrt_rn(__dmul_rn(-2.0, ln_unit33(w1)));
+    double c, s;
+    cos_sin_2pi32(w2, c, s);
+    z0 = __dmul_rn(R, c);
+    z1 = __dmul_rn(R, s);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Fast reciprocal square root / reciprocal in fp64: hardware seed (MUFU.RSQ64H / MUFU.RCP64H,
 // relative error <= ~2^-20) followed by ONE third-order correction, error ~ seed^3 < 2^-58.
 // Arguments here are always normal, positive and far from the exponent limits.

@@ -19,6 +19,7 @@ struct StateView {
     const GroupDev *groups;      // [n_groups]
     int32_t   W, N, ld;   // ld = N rounded up to a multiple of 4 (16-byte rows)
     uint32_t  walker_id_base;
+    int32_t   proposal;   // 0: particles in order, uniform cube (R7); 1: random particle, Gaussian step (l.144, l.325)
 };
 
 struct TraceView {

@@ -39,7 +39,9 @@ template <> struct ModeT<double> { using Coord = double;  using Disp = double; }
 template <> struct ModeT<float>  { using Coord = int32_t; using Disp = int32_t; };
 
 // Displacement (coordinate units, already times step) and log(xi) of one move.
-template <typename Real> struct MoveRand { double logxi; typename ModeT<Real>::Disp dx, dy, dz; };
+template <typename Real> struct MoveRand { double logxi; typename ModeT<Real>::Disp dx, dy, dz; int32_t s; };
+// bytes of one record in the shared-memory variate ring (16-byte aligned)
+template <typename Real> struct MoveSlot { static constexpr int bytes = (int)((sizeof(MoveRand<Real>) + 15) / 16 * 16); };
 
 // V consecutive values as one shared-memory vector access.
 template <typename E, int V> struct alignas(sizeof(E) * V) Pack { E v[V]; };
@@ -150,9 +152,10 @@ __device__ __forceinline__ int s_index(int j)
 static inline int sweep_smem_bytes(int T, int J, int mode, int P)
 {
     const int real = (mode == QMC_FP64) ? 8 : 4;
+    const int slot = (mode == QMC_FP64) ? MoveSlot<double>::bytes : MoveSlot<float>::bytes;
     const int NP = T * J;
     (void)P;                                             // hi + lo takes the room of the fp64 sums
-    return NP * 8 + 2 * kChunk * 32 + 64 * 8 + 3 * NP * real;
+    return NP * 8 + 2 * kChunk * slot + 64 * 8 + 3 * NP * real;
 }
 
 // Resident CTAs per SM the register allocator should leave room for: what shared memory allows for
@@ -161,7 +164,7 @@ template <typename Real, int T, int J, int P>
 constexpr int sweep_min_ctas()
 {
     const int real = (int)sizeof(Real);
-    const int smem = J * T * (8 + 3 * real) + 2 * kChunk * 32 + 64 * 8 + 1024;
+    const int smem = J * T * (8 + 3 * real) + 2 * kChunk * 48 + 64 * 8 + 1024;
     const int by_smem = (228 * 1024) / smem;
     const int regs = (real == 8 ? 96 + 3 * J : 40 + 3 * J);
     const int by_regs = 65536 / (regs * T);
@@ -214,7 +217,7 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
     using PackC = Pack<Coord, V>;
     constexpr bool kF32 = (sizeof(Real) == 4);
     constexpr bool kPacked = kF32 && V >= 2;              // two pair terms per FFMA2-class instruction
-    constexpr int NP = T * J, G = J / V, nwarps = T >> 5;
+    constexpr int NP = T * J, G = J / V, nwarps = T >> 5, kSlot = MoveSlot<Real>::bytes;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int N = sv.N, ld = sv.ld;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -222,11 +225,11 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
 
     double         *S    = reinterpret_cast<double *>(smem_raw);                              // [NP], permuted (s_index)
     unsigned char  *rnd  = smem_raw + NP * 8;                                                 // [2][kChunk] 32-byte slots
-    double         *part = reinterpret_cast<double *>(smem_raw + NP * 8 + 2 * kChunk * 32);   // [2][32]
+    double         *part = reinterpret_cast<double *>(smem_raw + NP * 8 + 2 * kChunk * kSlot);   // [2][32]
     Coord          *x    = reinterpret_cast<Coord *>(part + 64);                              // [3][NP]
     Coord *y = x + NP, *z = x + 2 * NP;
     float *Shi = reinterpret_cast<float *>(S), *Slo = Shi + NP;                               // PD = 1: S as hi + lo, [NP] each
-    static_assert(sizeof(MoveRand<Real>) <= 32, "variate record must fit its 32-byte slot");
+    static_assert(sizeof(MoveRand<Real>) <= kSlot, "variate record must fit its slot");
 
     const GroupDev g = sv.groups[sv.group_of[w]];
     SweepConst<Real> P;
@@ -276,12 +279,27 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
         const uint32_t m = chunk * kChunk + lane;
         if (m >= total) return;
         const uint32_t q = m / (uint32_t)N;
-        const uint32_t s = m - q * (uint32_t)N;
-        const uint4 r = philox4x32_10(make_uint4(s, t0 + q, wid, 0u), key);
+        const uint32_t idx = m - q * (uint32_t)N;
         MoveRand<Real> mr;
-        const double ax = __dmul_rn(step, word_to_pm1(r.x));
-        const double ay = __dmul_rn(step, word_to_pm1(r.y));
-        const double az = __dmul_rn(step, word_to_pm1(r.z));
+        double ax, ay, az;
+        uint32_t wxi;
+        if (DBG && sv.proposal == 1) {                     // random particle, Gaussian displacement (l.144, l.325)
+            const uint4 A = philox4x32_10(make_uint4(idx, t0 + q, wid, 2u), key);
+            const uint4 B = philox4x32_10(make_uint4(idx, t0 + q, wid, 3u), key);
+            mr.s = (int32_t)__umulhi(A.x, (uint32_t)N);
+            double z0, z1, z2, z3;
+            normal_pair(A.y, A.z, z0, z1);
+            normal_pair(B.x, B.y, z2, z3);
+            ax = __dmul_rn(step, z0); ay = __dmul_rn(step, z1); az = __dmul_rn(step, z2);
+            wxi = A.w;
+        } else {                                           // particles in order, uniform cube (R7)
+            const uint4 r = philox4x32_10(make_uint4(idx, t0 + q, wid, 0u), key);
+            mr.s = (int32_t)idx;
+            ax = __dmul_rn(step, word_to_pm1(r.x));
+            ay = __dmul_rn(step, word_to_pm1(r.y));
+            az = __dmul_rn(step, word_to_pm1(r.z));
+            wxi = r.w;
+        }
         if constexpr (kF32) {
             mr.dx = (int32_t)((uint32_t)__double2int_rn(ax) << 9);
             mr.dy = (int32_t)((uint32_t)__double2int_rn(ay) << 9);
@@ -289,11 +307,11 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
         } else {
             mr.dx = ax; mr.dy = ay; mr.dz = az;
         }
-        mr.logxi = log(word_to_unit(r.w));
-        *reinterpret_cast<MoveRand<Real> *>(rnd + (buf * kChunk + lane) * 32) = mr;
+        mr.logxi = log(word_to_unit(wxi));
+        *reinterpret_cast<MoveRand<Real> *>(rnd + (buf * kChunk + lane) * kSlot) = mr;
     };
     auto fetch = [&](uint32_t m) {
-        return *reinterpret_cast<const MoveRand<Real> *>(rnd + ((int)((m >> 5) & 1) * kChunk + (int)(m & (kChunk - 1))) * 32);
+        return *reinterpret_cast<const MoveRand<Real> *>(rnd + ((int)((m >> 5) & 1) * kChunk + (int)(m & (kChunk - 1))) * kSlot);
     };
     produce(0, 0);
     if (tid == 0) *reinterpret_cast<int32_t *>(part + 63) = 0;
@@ -301,9 +319,11 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
     const int32_t zero = opaque_zero(reinterpret_cast<int32_t *>(part + 63));   // part[32..63] is used from move 1 on
 
     unsigned long long n_acc = 0;
-    int s = 0;
     MoveRand<Real> mr = fetch(0);
-    Coord xs = x[0], ys = y[0], zs = z[0];                 // the moved particle (prefetched one move ahead)
+    int s = DBG ? mr.s : 0;
+    Coord xs = x[s], ys = y[s], zs = z[s];                 // the moved particle (prefetched one move ahead)
+    int sp = -1;                                           // DBG: particle of the previous move and where it ended up
+    Coord pxp = xs, pyp = ys, pzp = zs;
     __syncthreads();                                       // ... before its owner poisons it
     for (uint32_t m = 0; m < total; ++m) {
         if ((m & (kChunk - 1)) == 0) produce((m >> 5) + 1, (int)(((m >> 5) + 1) & 1));   // published by this move's barrier
@@ -314,10 +334,16 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
         const bool owner = ((unsigned)tid == (((unsigned)s / (unsigned)V) & (unsigned)(T - 1)));
         if (owner) x[s] = poison_of<Real>(tx);             // self term = 0 (nobody else reads x[s] during this move)
 
-        // prefetch the next move: its particle cannot change in this move (N >= 3; else re-read below)
-        const int sn = (s + 1 == N) ? 0 : s + 1;
-        const Coord xn = x[sn], yn = y[sn], zn = z[sn];
-        if (m + 1 < total) mr = fetch(m + 1);
+        // prefetch the next move.  Lean kernel: particles in order, N >= 3 -- the next particle is touched
+        // neither by this move nor by the previous one.  DBG kernel (any N, random particle): the next
+        // particle may be this move's (resolved after the decision) or the previous move's (whose commit
+        // by its owner is not ordered against this read: every thread kept the outcome in registers).
+        MoveRand<Real> mrn = mr;
+        if (m + 1 < total) mrn = fetch(m + 1);
+        int sn;
+        if constexpr (DBG) sn = mrn.s; else sn = (s + 1 == N) ? 0 : s + 1;
+        Coord xn = x[sn], yn = y[sn], zn = z[sn];
+        if constexpr (DBG) { if (sn == sp) { xn = pxp; yn = pyp; zn = pzp; } }
 
         // a3: trial terms of this thread's particles
         Real un[kPacked ? 1 : J];
@@ -472,13 +498,16 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
                 }
             }
         }
+        if constexpr (DBG) {
+            const Coord cx = accept ? commit_coord(tx, g.L) : xs;
+            const Coord cy = accept ? commit_coord(ty, g.L) : ys;
+            const Coord cz = accept ? commit_coord(tz, g.L) : zs;
+            if (sn == s) { xn = cx; yn = cy; zn = cz; }
+            sp = s; pxp = cx; pyp = cy; pzp = cz;
+        }
         s = sn;
         xs = xn; ys = yn; zs = zn;
-        if (DBG && N < 3) {                                 // degenerate: the next particle may just have moved
-            __syncthreads();
-            xs = x[s]; ys = y[s]; zs = z[s];
-            __syncthreads();
-        }
+        mr = mrn;
     }
     __syncthreads();
 
@@ -503,8 +532,8 @@ template <typename Real, int T, int J, int V, int PD>
 static cudaError_t shape_launch(qmc_ctx *c, int n_sweeps, int smem)
 {
     const uint2 key = make_uint2((uint32_t)(c->seed & 0xFFFFFFFFull), (uint32_t)(c->seed >> 32));
-    // the lean instantiation has neither the decision trace nor the N < 3 re-read of the next particle
-    const bool dbg = c->trace.dec != nullptr || c->p.N < 3;
+    // the lean instantiation has neither the decision trace nor the general next-particle handling (N < 3, proposal 1)
+    const bool dbg = c->trace.dec != nullptr || c->p.N < 3 || c->sv.proposal != 0;
     auto kern = dbg ? sweep_kernel<Real, T, J, V, PD, true> : sweep_kernel<Real, T, J, V, PD, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;

@@ -489,3 +489,70 @@ def test_reblock_recovers_the_error_of_an_ar1_series():
     assert 0.8 < se2 * math.sqrt(4096) < 1.35 and tau2 < 1.0
     tsig, t_goal = ob.seconds_to_error(2e-3, 10.0)
     assert abs(tsig - 40.0) < 1e-9 and abs(t_goal - 40.0) < 1e-9
+
+
+# ------------------------------------------------------------------ proposal 1: random particle, Gaussian step (NEXT-1)
+def test_normal_variates_match_the_library_functions(oracle):
+    """The bit-specified Box-Muller (own ln, cos, sin from +,-,*,/,sqrt) against math.log / cos / sin."""
+    rng = np.random.default_rng(17)
+    words = [0, 1, 2, 2**30 - 1, 2**30, 2**31, 3 * 2**30 + 5, 2**32 - 1] + [int(v) for v in rng.integers(0, 2**32, 300)]
+    for w1 in words[:40]:
+        for w2 in words:
+            z0, z1 = oracle.normal_pair(w1, w2)
+            R = math.sqrt(-2.0 * math.log((2 * w1 + 1) / 2.0**33))
+            a = 2.0 * math.pi * (w2 + 0.5) / 2.0**32
+            assert abs(z0 - R * math.cos(a)) < 4e-15 * max(1.0, R) and abs(z1 - R * math.sin(a)) < 4e-15 * max(1.0, R)
+    assert abs(oracle.normal_pair(0, 0)[0] - math.sqrt(66 * math.log(2.0))) < 1e-8      # largest |z|: 6.7637...
+
+
+def test_normal_variates_are_standard_normal(oracle):
+    """Moments and a Kolmogorov-Smirnov distance of 2 x 40000 variates drawn through Philox words."""
+    from scipy import stats
+    z = []
+    for m in range(20000):
+        _, d, _ = oracle.move_variates_gauss(99, 3, 1, m, 1000, 1.0)
+        z.append(d)
+    z = np.array(z)
+    assert np.all(np.abs(z.mean(0)) < 4.5 / math.sqrt(len(z)))
+    assert np.all(np.abs(z.var(0) - 1.0) < 4.5 * math.sqrt(2.0 / len(z)))
+    assert np.all(np.abs((z ** 4).mean(0) - 3.0) < 4.5 * math.sqrt(96.0 / len(z)))
+    c = np.corrcoef(z.T)
+    assert abs(c[0, 1]) < 0.04 and abs(c[0, 2]) < 0.04 and abs(c[1, 2]) < 0.04
+    for k in range(3):
+        assert stats.kstest(z[:, k], "norm").pvalue > 1e-4
+    # scaling by step is one multiplication; the particle index is uniform over 0..N-1
+    s1, d1, xi1 = oracle.move_variates_gauss(99, 3, 1, 7, 1000, 1.0)
+    s2, d2, xi2 = oracle.move_variates_gauss(99, 3, 1, 7, 1000, 0.37)
+    assert s1 == s2 and xi1 == xi2 and np.array_equal(d2, 0.37 * d1)
+    idx = np.array([oracle.move_variates_gauss(5, 0, 0, m, 10, 1.0)[0] for m in range(20000)])
+    cnt = np.bincount(idx, minlength=10)
+    assert idx.min() == 0 and idx.max() == 9 and np.all(np.abs(cnt - 2000) < 5 * math.sqrt(2000))
+
+
+def test_proposal1_samples_psi_squared_for_two_atoms(oracle):
+    """P5 under proposal 1: N = 2 in a small box, sampled minimum-image pair distance against brute-force
+    quadrature of |psi|^2 over the cube (a proposal that broke detailed balance would fail this)."""
+    L, b, nb = 8.0, 2.89, 24
+    s = oracle.System(2, L, b, DK, AZ, proposal=1)
+    W, sweeps = 16, 3000
+    xyz = oracle.init_walkers(s, 3, 0, W, 0.05)
+    oracle.sweep(s, xyz, 3, 0, 0, 200, 0.5)
+    rmax = L * math.sqrt(3.0) / 2.0
+    hist = np.zeros(nb)
+    t = 200
+    for _ in range(sweeps // 10):
+        oracle.sweep(s, xyz, 3, 0, t, 10, 0.5)
+        t += 10
+        d = xyz[:, :, 0] - xyz[:, :, 1]
+        d -= L * np.rint(d / L)
+        r = np.sqrt((d ** 2).sum(1))
+        hist += np.histogram(r, bins=nb, range=(0.0, rmax))[0]
+    hist /= hist.sum()
+    g = (np.arange(60) + 0.5) / 60 * L - L / 2
+    X, Y, Z = np.meshgrid(g, g, g, indexing="ij")
+    R = np.sqrt(X ** 2 + Y ** 2 + Z ** 2).ravel()
+    wgt = np.array([math.exp(2.0 * oracle.u(r, L, b)) for r in R])
+    ref = np.histogram(R, bins=nb, range=(0.0, rmax), weights=wgt)[0]
+    ref /= ref.sum()
+    n_eff = W * (sweeps // 10) / 4.0
+    assert np.all(np.abs(hist - ref) < 5.0 * np.sqrt(ref * (1 - ref) / n_eff) + 4e-3), np.abs(hist - ref).max()
