@@ -14,8 +14,8 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqmc_b200.so")
-SOURCES = ["qmc_api.cu", "qmc_sweep_plan.cu", "qmc_sweep_f32.cu", "qmc_sweep_f64.cu", "qmc_energy.cu", "qmc_energy_f32.cu", "qmc_energy_f64.cu", "qmc_observables.cu"]
-HEADERS = ["qmc_device.cuh", "qmc_internal.h", "qmc_sweep_impl.cuh", "qmc_f32c.cuh", os.path.join("..", "..", "include", "qmc.h")]
+SOURCES = ["qmc_api.cu", "qmc_sweep_plan.cu", "qmc_sweep_f32.cu", "qmc_sweep_f64.cu", "qmc_energy.cu", "qmc_energy_f32.cu", "qmc_energy_f32s.cu", "qmc_energy_f64.cu", "qmc_observables.cu"]
+HEADERS = ["qmc_device.cuh", "qmc_internal.h", "qmc_sweep_impl.cuh", "qmc_f32c.cuh", "qmc_energy_f32_pair.cuh", os.path.join("..", "..", "include", "qmc.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]

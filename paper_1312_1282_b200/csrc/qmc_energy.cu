@@ -242,7 +242,9 @@ static cudaError_t launch_e(qmc_ctx *c, double *d_out, bool energy)
 cudaError_t launch_energy(qmc_ctx *c, double *d_out, bool energy)
 {
     c->launches += 1;
-    if (c->p.mode != QMC_FP64) return launch_energy_f32(c, d_out, energy);     // qmc_energy_f32.cu
+    if (c->p.mode != QMC_FP64)
+        return c->energy_plan.variant == 2 ? launch_energy_f32s(c, d_out, energy)    // qmc_energy_f32s.cu
+                                           : launch_energy_f32(c, d_out, energy);    // qmc_energy_f32.cu
     if (c->energy_plan.variant == 1) return launch_energy_f64(c, d_out, energy);  // qmc_energy_f64.cu
     const int T = c->energy_plan.threads;
 #define X(TT) if (T == TT) return launch_e<double, TT>(c, d_out, energy);
@@ -254,7 +256,11 @@ cudaError_t launch_energy(qmc_ctx *c, double *d_out, bool energy)
 bool plan_energy(qmc_ctx *c, EnergyPlan *out)
 {
     out->variant = 0;
-    if (c->p.mode != QMC_FP64) return plan_energy_f32(c, out);
+    if (c->p.mode != QMC_FP64) {
+        if (!getenv("QMC_ENERGY_ORDERED") && plan_energy_f32s(c, out)) return true;
+        out->variant = 0;
+        return plan_energy_f32(c, out);
+    }
     if (!getenv("QMC_ENERGY_ORDERED") && plan_energy_f64(c, out)) return true;
     out->variant = 0;
     const int N = c->p.N;

@@ -73,6 +73,8 @@ bool plan_sweep(qmc_ctx *c, SweepPlan *out);
 bool plan_energy(qmc_ctx *c, EnergyPlan *out);
 cudaError_t launch_energy_f32(qmc_ctx *c, double *d_out, bool energy);
 bool plan_energy_f32(qmc_ctx *c, EnergyPlan *out);
+cudaError_t launch_energy_f32s(qmc_ctx *c, double *d_out, bool energy);   // unordered pairs (qmc_energy_f32s.cu)
+bool plan_energy_f32s(qmc_ctx *c, EnergyPlan *out);
 cudaError_t launch_energy_f64(qmc_ctx *c, double *d_out, bool energy);
 bool plan_energy_f64(qmc_ctx *c, EnergyPlan *out);
 
