@@ -14,7 +14,8 @@
  *
  * Citations are PAPER.md line numbers (arxiv 1312.1282) and DESIGN.md readings
  * R1..R21.  Parity pins: tests/test_oracle_pins.py (every function below is
- * pinned there; nothing in this file is "parity unpinned").
+ * pinned there, including the proposal-1 variates and the pair histogram;
+ * nothing in this file is "parity unpinned").
  */
 #include <math.h>
 #include <stdint.h>
