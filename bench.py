@@ -330,6 +330,23 @@ def main():
         ms = e0.elapsed_time(e1) / 3
         out["observables"] = {"pair_histogram_ms": ms, "pairs_per_s": W * N * (N - 1) / 2 / (ms * 1e-3), "nbins": nb,
                               "pairs_inside_cutoff_per_walker": float(hist.sum(1).double().mean())}
+    # ---- NEXT-4: blocks with in-flight write-outs (state stays on the device, results stream to pinned host memory)
+    nblk = max(3, min(K, 10))
+    hb_e = torch.zeros((nblk, W, 4), dtype=torch.float64).pin_memory()
+    hb_a = torch.zeros((nblk, W), dtype=torch.float64).pin_memory()
+    hb_d = torch.zeros((nblk,), dtype=torch.int32).pin_memory()
+    q.run_blocks_host(1, m, steps, hb_e, hb_a, hb_d)
+    q.wait()
+    hb_d.zero_()
+    t0 = time.perf_counter()
+    q.run_blocks_host(nblk, m, steps, hb_e, hb_a, hb_d)
+    t_enq = time.perf_counter() - t0
+    q.wait()
+    t_blk = time.perf_counter() - t0
+    out["blocks_host"] = {"value": nblk * pairs_step / t_blk, "unit": "pair-evals/s", "blocks": nblk,
+                          "ms_per_block": 1e3 * t_blk / nblk, "enqueue_ms": 1e3 * t_enq,
+                          "d2h_bytes_per_block": W * 5 * 8, "flags_raised": int(hb_d.sum()),
+                          "api": "qmc_run_blocks_host (write-outs on a second stream while the next block computes)"}
     if args.time_to_error > 0:
         from paper_1312_1282_b200 import observables as ob
         S = args.time_to_error

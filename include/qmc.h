@@ -115,6 +115,17 @@ int qmc_acceptance(qmc_ctx *c, double *d_out);
 int qmc_step_host(qmc_ctx *c, const double *h_xyz_in, int32_t n_sweeps, const double *steps,
                   double *h_energy, double *h_acc, double *h_xyz_out);
 
+/* A run of n_blocks blocks with in-flight write-outs (the paper's load masking, l.175, l.323, §4; SURVEY.md §8(f)
+ * NEXT-4).  Block b = sweeps_per_block sweeps + local energy + acceptance; its results go to the HOST arrays
+ * h_energy[b][W][4] and h_acc[b][W] (may be NULL) on a second stream while block b+1 computes, and h_done[b]
+ * (host int32, may be NULL; the caller zeroes it) is set to 1 once they have landed, so the host can analyse
+ * block b while the GPU generates the next ones.  Use pinned host memory.  Returns after ENQUEUEING all blocks;
+ * qmc_wait (or polling h_done[n_blocks-1]) tells when everything is there.  The buffers must stay valid until then. */
+int qmc_run_blocks_host(qmc_ctx *c, int32_t n_blocks, int32_t sweeps_per_block, const double *steps,
+                        double *h_energy, double *h_acc, int32_t *h_done);
+/* Blocks until all work of this context (both streams) has finished. */
+int qmc_wait(qmc_ctx *c);
+
 /* Message for the last error of this context (or of the last failed qmc_create if c is NULL).
  * Library-owned, valid until the next call. */
 const char *qmc_last_error(const qmc_ctx *c);

@@ -21,7 +21,7 @@ EXPORTS = (
     "qmc_state_bytes", "qmc_create", "qmc_destroy", "qmc_init_walkers", "qmc_sweep", "qmc_local_energy",
     "qmc_acceptance", "qmc_step_host", "qmc_last_error", "qmc_get_positions", "qmc_set_positions",
     "qmc_set_seed", "qmc_get_pair_sums", "qmc_refresh_pair_sums", "qmc_trace_decisions", "qmc_info",
-    "qmc_pipe_peak", "qmc_pair_histogram", "qmc_set_proposal",
+    "qmc_pipe_peak", "qmc_pair_histogram", "qmc_set_proposal", "qmc_run_blocks_host", "qmc_wait",
 )
 
 
@@ -79,6 +79,8 @@ def load_library() -> C.CDLL:
     lib.qmc_acceptance.argtypes = [vp, vp]
     lib.qmc_pair_histogram.argtypes = [vp, C.c_int32, vp]
     lib.qmc_set_proposal.argtypes = [vp, C.c_int32]
+    lib.qmc_run_blocks_host.argtypes = [vp, C.c_int32, C.c_int32, dp, vp, vp, vp]
+    lib.qmc_wait.argtypes = [vp]
     lib.qmc_step_host.argtypes = [vp, vp, C.c_int32, dp, vp, vp, vp]
     lib.qmc_last_error.argtypes = [vp]
     lib.qmc_last_error.restype = C.c_char_p
@@ -215,6 +217,19 @@ class QMC:
             out = torch.empty((self.W,), dtype=torch.float64, device=self.device)
         self._check(self._lib.qmc_acceptance(self._ctx, self._ptr(out, torch.float64, self.W)))
         return out
+
+    def run_blocks_host(self, n_blocks: int, sweeps_per_block: int, steps, h_energy, h_acc=None, h_done=None):
+        """qmc_run_blocks_host: asynchronous; h_energy [n_blocks][W][4], h_acc [n_blocks][W] float64 and
+        h_done [n_blocks] int32 are pinned host tensors that must stay alive until wait()."""
+        torch = self._torch
+        self._check(self._lib.qmc_run_blocks_host(
+            self._ctx, int(n_blocks), int(sweeps_per_block), self._steps(steps),
+            self._ptr(h_energy, torch.float64, n_blocks * self.W * 4, "cpu"),
+            self._ptr(h_acc, torch.float64, n_blocks * self.W, "cpu") if h_acc is not None else None,
+            self._ptr(h_done, torch.int32, n_blocks, "cpu") if h_done is not None else None))
+
+    def wait(self):
+        self._check(self._lib.qmc_wait(self._ctx))
 
     def set_proposal(self, kind: int):
         """0: particles in order, uniform cube; 1: random particle, Gaussian displacement (qmc.h)."""

@@ -350,6 +350,13 @@ extern "C" int qmc_destroy(qmc_ctx *c)
     if (c->d_groups) cudaFree(c->d_groups);
     if (c->d_group_of) cudaFree(c->d_group_of);
     if (c->d_scratch) cudaFree(c->d_scratch);
+    if (c->out_stream) cudaStreamSynchronize(c->out_stream);
+    if (c->d_block) cudaFree(c->d_block);
+    for (int k = 0; k < 2; ++k) {
+        if (c->ev_ready[k]) cudaEventDestroy(c->ev_ready[k]);
+        if (c->ev_copied[k]) cudaEventDestroy(c->ev_copied[k]);
+    }
+    if (c->out_stream) cudaStreamDestroy(c->out_stream);
     delete c;
     return QMC_OK;
 }
@@ -517,6 +524,52 @@ extern "C" int qmc_step_host(qmc_ctx *c, const double *h_xyz_in, int32_t n_sweep
         QMC_CUDA(c, cudaMemcpyAsync(h_xyz_out, d_x, sizeof(double) * W * 3 * N, cudaMemcpyDeviceToHost, c->stream));
     }
     QMC_CUDA(c, cudaStreamSynchronize(c->stream));
+    return QMC_OK;
+}
+
+// Host function of the write-out stream: the block's data have landed, raise its flag.
+static void CUDART_CB raise_flag(void *flag) { *reinterpret_cast<volatile int32_t *>(flag) = 1; }
+
+extern "C" int qmc_run_blocks_host(qmc_ctx *c, int32_t n_blocks, int32_t sweeps_per_block, const double *steps,
+                                   double *h_energy, double *h_acc, int32_t *h_done)
+{
+    if (!c || !h_energy) return QMC_E_ARG;
+    if (!c->have_state) QMC_FAIL(c, QMC_E_STATE, "qmc_run_blocks_host before qmc_init_walkers / qmc_set_positions");
+    if (n_blocks < 0 || sweeps_per_block < 1) QMC_FAIL(c, QMC_E_ARG, "n_blocks >= 0 and sweeps_per_block >= 1 required");
+    const size_t W = (size_t)c->W;
+    if (!c->out_stream) {
+        QMC_CUDA(c, cudaStreamCreateWithFlags(&c->out_stream, cudaStreamNonBlocking));
+        QMC_CUDA(c, cudaMalloc(&c->d_block, sizeof(double) * 2 * W * 5));
+        for (int k = 0; k < 2; ++k) {
+            QMC_CUDA(c, cudaEventCreateWithFlags(&c->ev_ready[k], cudaEventDisableTiming));
+            QMC_CUDA(c, cudaEventCreateWithFlags(&c->ev_copied[k], cudaEventDisableTiming));
+        }
+    }
+    for (int32_t b = 0; b < n_blocks; ++b) {
+        const int k = b & 1;
+        double *d_e = c->d_block + (size_t)k * W * 5, *d_a = d_e + 4 * W;
+        int rc = qmc_sweep(c, sweeps_per_block, steps);
+        if (rc != QMC_OK) return rc;
+        if (b >= 2) QMC_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copied[k], 0));   // buffer k is free again
+        if ((rc = qmc_local_energy(c, d_e)) != QMC_OK) return rc;
+        if ((rc = qmc_acceptance(c, d_a)) != QMC_OK) return rc;
+        QMC_CUDA(c, cudaEventRecord(c->ev_ready[k], c->stream));
+        // write-out while the next block computes (the paper's asynchronous writeouts, l.175, l.323)
+        QMC_CUDA(c, cudaStreamWaitEvent(c->out_stream, c->ev_ready[k], 0));
+        QMC_CUDA(c, cudaMemcpyAsync(h_energy + (size_t)b * W * 4, d_e, sizeof(double) * 4 * W, cudaMemcpyDeviceToHost, c->out_stream));
+        if (h_acc)
+            QMC_CUDA(c, cudaMemcpyAsync(h_acc + (size_t)b * W, d_a, sizeof(double) * W, cudaMemcpyDeviceToHost, c->out_stream));
+        QMC_CUDA(c, cudaEventRecord(c->ev_copied[k], c->out_stream));
+        if (h_done) QMC_CUDA(c, cudaLaunchHostFunc(c->out_stream, raise_flag, h_done + b));
+    }
+    return QMC_OK;
+}
+
+extern "C" int qmc_wait(qmc_ctx *c)
+{
+    if (!c) return QMC_E_ARG;
+    QMC_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->out_stream) QMC_CUDA(c, cudaStreamSynchronize(c->out_stream));
     return QMC_OK;
 }
 

@@ -47,6 +47,10 @@ struct qmc_ctx {
     qmc::GroupDev *d_groups = nullptr;
     int32_t *d_group_of = nullptr;
     double *d_scratch = nullptr;                   // [W][4] + [W] + [W][3][N] staging for *_host calls
+    // qmc_run_blocks_host: write-out stream, double-buffered block results, their events (created on first use)
+    cudaStream_t out_stream = nullptr;
+    double *d_block = nullptr;                     // [2][W][5]
+    cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
     qmc::TraceView trace{};
     qmc::SweepPlan sweep_plan{};
     qmc::EnergyPlan energy_plan{};

@@ -464,6 +464,29 @@ def test_step_host_equals_device_calls(qmc):
         assert torch.equal(q2.get_positions().cpu(), h_x)
 
 
+def test_run_blocks_host_equals_stepwise_calls(qmc):
+    """qmc_run_blocks_host (NEXT-4: blocks with in-flight write-outs on a second stream) against the same
+    sequence of qmc_sweep / qmc_local_energy / qmc_acceptance calls: identical numbers, flags raised."""
+    import torch
+    N, W, blocks, m = 100, 5, 7, 2
+    for mode in (qmc.QMC_FP64, qmc.QMC_FP32C):
+        qa, _ = make(qmc, N, W, mode)
+        qb, _ = make(qmc, N, W, mode)
+        qa.init_walkers(3)
+        qb.init_walkers(3)
+        he = torch.zeros((blocks, W, 4), dtype=torch.float64).pin_memory()
+        ha = torch.zeros((blocks, W), dtype=torch.float64).pin_memory()
+        hd = torch.zeros((blocks,), dtype=torch.int32).pin_memory()
+        qa.run_blocks_host(blocks, m, 1.0, he, ha, hd)
+        qa.wait()
+        assert hd.tolist() == [1] * blocks
+        for b in range(blocks):
+            qb.sweep(m, 1.0)
+            assert np.array_equal(qb.local_energy().cpu().numpy(), he[b].numpy())
+            assert np.array_equal(qb.acceptance().cpu().numpy(), ha[b].numpy())
+        assert torch.equal(qa.get_positions(), qb.get_positions())
+
+
 def test_pipe_peak_microbenchmark_is_plausible(qmc):
     f64 = qmc.pipe_peak(0)
     f32 = qmc.pipe_peak(1)
