@@ -117,12 +117,27 @@ int qmc_step_host(qmc_ctx *c, const double *h_xyz_in, int32_t n_sweeps, const do
 
 /* A run of n_blocks blocks with in-flight write-outs (the paper's load masking, l.175, l.323, §4; SURVEY.md §8(f)
  * NEXT-4).  Block b = sweeps_per_block sweeps + local energy + acceptance; its results go to the HOST arrays
- * h_energy[b][W][4] and h_acc[b][W] (may be NULL) on a second stream while block b+1 computes, and h_done[b]
- * (host int32, may be NULL; the caller zeroes it) is set to 1 once they have landed, so the host can analyse
- * block b while the GPU generates the next ones.  Use pinned host memory.  Returns after ENQUEUEING all blocks;
- * qmc_wait (or polling h_done[n_blocks-1]) tells when everything is there.  The buffers must stay valid until then. */
+ * h_energy[b][W][4] and h_acc[b][W] (may be NULL) on a second stream while block b+1 computes.  If h_xyz is not
+ * NULL, every xyz_every-th block (b+1 a multiple of xyz_every >= 1) also writes the walker coordinates out, to
+ * h_xyz[(b+1)/xyz_every - 1][W][3][N] (l.323: "walker coordinates ... acceptance ratio, computed potential and
+ * kinetic energies").  h_done[b] (host int32, may be NULL; the caller zeroes it) is set to 1 once everything of
+ * block b has landed, so the host can analyse block b while the GPU generates the next ones.  Use pinned host
+ * memory.  Returns after ENQUEUEING all blocks; qmc_wait (or polling h_done[n_blocks-1]) tells when everything is
+ * there.  The buffers must stay valid until then.  Calls may follow each other without qmc_wait in between. */
 int qmc_run_blocks_host(qmc_ctx *c, int32_t n_blocks, int32_t sweeps_per_block, const double *steps,
-                        double *h_energy, double *h_acc, int32_t *h_done);
+                        double *h_energy, double *h_acc, int32_t xyz_every, double *h_xyz, int32_t *h_done);
+
+/* qmc_sweep with write-outs issued from INSIDE the running kernel (the paper's mechanism itself, l.175, l.323,
+ * l.343, Fig. 2; NEXT-4): the walker stays resident in shared memory for all n_sweeps sweeps of the ONE launch, and
+ * after every `every` sweeps (m of Fig. 2) each thread block writes its walker's coordinates to
+ * xyz_out[k][w][3][N] (Angstrom, k = 0 .. n_sweeps/every - 1) and its accepted-move count since init /
+ * set_positions to n_acc_out[k][w] (may be NULL), makes them visible system-wide, and sets flags[k][w] = 1 (the
+ * caller zeroes flags first).  The three buffers must be addressable by the device: device memory, or page-locked
+ * host memory mapped into the device address space (cudaHostAlloc / torch pin_memory: then the host sees each
+ * write-out while the kernel is still running and can analyse it -- the paper's load masking).  Asynchronous like
+ * qmc_sweep; the buffers must stay valid until the stream has finished. */
+int qmc_sweep_writeouts(qmc_ctx *c, int32_t n_sweeps, const double *steps, int32_t every,
+                        double *xyz_out, uint64_t *n_acc_out, int32_t *flags);
 /* Blocks until all work of this context (both streams) has finished. */
 int qmc_wait(qmc_ctx *c);
 
@@ -152,14 +167,21 @@ typedef struct {
     int32_t sm_count;
     uint32_t t;                       /* sweeps done since init                        */
     uint64_t kernel_launches;         /* kernels this context has launched so far      */
+    int32_t sweep_vector;             /* particles per shared-memory vector access (V) */
+    int32_t sweep_pending;            /* 1: running sums held as fp32 hi + lo (R20)    */
+    int32_t sweep_tile;               /* moves per barrier (K; 1 = one-move kernel)    */
+    int32_t energy_variant;           /* 0 ordered pairs, 1 fp64 / 2 fp32c unordered pairs, 3 gridded (large N) */
+    int32_t sweep_cluster;            /* thread blocks per walker (1; > 1: cluster kernel, distributed shared memory) */
 } qmc_info_t;
 int qmc_info(const qmc_ctx *c, qmc_info_t *out);
 
-/* Instruction-rate microbenchmark: runs a dependent-chain-free kernel of ONE
- * instruction kind on every SM and reports thread-level instructions per second (host out, synchronous).
- * which: 0 = fp64 DFMA, 1 = fp32 FFMA, 2 = packed FFMA2 (fma.rn.f32x2; two FMAs per instruction),
- * 3 = MUFU.RSQ (fp32 rsqrt.approx), 4 = I2FP (s32 -> f32), 5 = F2F (f64 -> f32 -> f64, both counted). */
-int qmc_pipe_peak(int32_t which, void *cuda_stream, double *h_fma_per_s);
+/* Process-wide override of the launch heuristics for the contexts created AFTERWARDS (tuning experiments and
+ * tests; the defaults are what bench.py times).  Keys: "sweep_threads", "sweep_per_thread", "sweep_vector",
+ * "sweep_pending", "sweep_tile" (1 = one-move kernel, 2 / 4 = tile kernel), "sweep_cluster", "energy_threads",
+ * "energy_ordered" (1 = ordered-pair energy kernels).  value: the wanted number, or -1 (0 for the energy keys) for
+ * "heuristic".  key == NULL resets everything.  A shape that is not compiled or does not fit N falls back to the
+ * heuristic.  Returns QMC_E_ARG for an unknown key. */
+int qmc_set_tuning(const char *key, int32_t value);
 
 #ifdef __cplusplus
 }

@@ -21,8 +21,10 @@ EXPORTS = (
     "qmc_state_bytes", "qmc_create", "qmc_destroy", "qmc_init_walkers", "qmc_sweep", "qmc_local_energy",
     "qmc_acceptance", "qmc_step_host", "qmc_last_error", "qmc_get_positions", "qmc_set_positions",
     "qmc_set_seed", "qmc_get_pair_sums", "qmc_refresh_pair_sums", "qmc_trace_decisions", "qmc_info",
-    "qmc_pipe_peak", "qmc_pair_histogram", "qmc_set_proposal", "qmc_run_blocks_host", "qmc_wait",
+    "qmc_pair_histogram", "qmc_set_proposal", "qmc_run_blocks_host", "qmc_wait", "qmc_sweep_writeouts",
+    "qmc_set_tuning",
 )
+PROBE_LIB_PATH = os.path.join(HERE, "libqmc_probe_b200.so")
 
 
 class QmcError(RuntimeError):
@@ -48,6 +50,8 @@ class Info(C.Structure):
         ("sweep_pairs_per_thread", C.c_int32),
         ("energy_threads", C.c_int32), ("energy_ctas_per_sm", C.c_int32), ("energy_smem_bytes", C.c_int32),
         ("sm_count", C.c_int32), ("t", C.c_uint32), ("kernel_launches", C.c_uint64),
+        ("sweep_vector", C.c_int32), ("sweep_pending", C.c_int32), ("sweep_tile", C.c_int32),
+        ("energy_variant", C.c_int32), ("sweep_cluster", C.c_int32),
     ]
 
     def as_dict(self):
@@ -79,7 +83,9 @@ def load_library() -> C.CDLL:
     lib.qmc_acceptance.argtypes = [vp, vp]
     lib.qmc_pair_histogram.argtypes = [vp, C.c_int32, vp]
     lib.qmc_set_proposal.argtypes = [vp, C.c_int32]
-    lib.qmc_run_blocks_host.argtypes = [vp, C.c_int32, C.c_int32, dp, vp, vp, vp]
+    lib.qmc_run_blocks_host.argtypes = [vp, C.c_int32, C.c_int32, dp, vp, vp, C.c_int32, vp, vp]
+    lib.qmc_sweep_writeouts.argtypes = [vp, C.c_int32, dp, C.c_int32, vp, vp, vp]
+    lib.qmc_set_tuning.argtypes = [C.c_char_p, C.c_int32]
     lib.qmc_wait.argtypes = [vp]
     lib.qmc_step_host.argtypes = [vp, vp, C.c_int32, dp, vp, vp, vp]
     lib.qmc_last_error.argtypes = [vp]
@@ -91,7 +97,6 @@ def load_library() -> C.CDLL:
     lib.qmc_refresh_pair_sums.argtypes = [vp]
     lib.qmc_trace_decisions.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, C.c_int64]
     lib.qmc_info.argtypes = [vp, C.POINTER(Info)]
-    lib.qmc_pipe_peak.argtypes = [C.c_int32, vp, dp]
     for name in EXPORTS:
         if name not in ("qmc_state_bytes", "qmc_last_error"):
             getattr(lib, name).restype = C.c_int
@@ -108,17 +113,36 @@ def _make_params(N, walkers_per_group, box_L, jastrow_b, hbar2_over_2m, aziz, mo
     return p, keep
 
 
+_probe = None
+
+
 def pipe_peak(which: int, stream=None) -> float:
-    """Thread-level instructions per second of one instruction kind, measured live (qmc.h: 0 DFMA,
-    1 FFMA, 2 FFMA2, 3 MUFU.RSQ, 4 I2FP, 5 F2F)."""
+    """Thread-level instructions per second of one instruction kind, measured live by the separate probe library
+    (include/qmc_probe.h: 0 DFMA, 1 FFMA, 2 FFMA2, 3 MUFU.RSQ, 4 I2FP, 5 F2F)."""
     import torch
-    lib = load_library()
+    global _probe
+    if _probe is None:
+        if not os.path.exists(PROBE_LIB_PATH):
+            raise FileNotFoundError(f"{PROBE_LIB_PATH} is missing: python -m paper_1312_1282_b200.build")
+        _probe = C.CDLL(PROBE_LIB_PATH)
+        _probe.qmc_probe_rate.argtypes = [C.c_int32, C.c_void_p, C.POINTER(C.c_double)]
+        _probe.qmc_probe_rate.restype = C.c_int
+    if not torch.cuda.is_available():
+        raise QmcError(QMC_E_CUDA, "no CUDA device")
     st = torch.cuda.current_stream() if stream is None else stream
     out = C.c_double()
-    rc = lib.qmc_pipe_peak(which, C.c_void_p(st.cuda_stream), C.byref(out))
+    rc = _probe.qmc_probe_rate(which, C.c_void_p(st.cuda_stream), C.byref(out))
+    if rc != 0:
+        raise QmcError(rc, "qmc_probe_rate failed")
+    return out.value
+
+
+def set_tuning(key: Optional[str] = None, value: int = -1):
+    """qmc_set_tuning: process-wide launch-heuristic override for contexts created afterwards; set_tuning() resets."""
+    lib = load_library()
+    rc = lib.qmc_set_tuning(key.encode() if key is not None else None, int(value))
     if rc != 0:
         raise QmcError(rc, lib.qmc_last_error(None).decode())
-    return out.value
 
 
 class QMC:
@@ -218,15 +242,33 @@ class QMC:
         self._check(self._lib.qmc_acceptance(self._ctx, self._ptr(out, torch.float64, self.W)))
         return out
 
-    def run_blocks_host(self, n_blocks: int, sweeps_per_block: int, steps, h_energy, h_acc=None, h_done=None):
-        """qmc_run_blocks_host: asynchronous; h_energy [n_blocks][W][4], h_acc [n_blocks][W] float64 and
-        h_done [n_blocks] int32 are pinned host tensors that must stay alive until wait()."""
+    def run_blocks_host(self, n_blocks: int, sweeps_per_block: int, steps, h_energy, h_acc=None, h_done=None,
+                        xyz_every: int = 0, h_xyz=None):
+        """qmc_run_blocks_host: asynchronous; h_energy [n_blocks][W][4], h_acc [n_blocks][W] float64, h_done [n_blocks]
+        int32 and h_xyz [n_blocks // xyz_every][W][3][N] float64 are pinned host tensors that must stay alive until wait()."""
         torch = self._torch
+        n_xyz = (n_blocks // xyz_every) if (h_xyz is not None and xyz_every > 0) else 0
         self._check(self._lib.qmc_run_blocks_host(
             self._ctx, int(n_blocks), int(sweeps_per_block), self._steps(steps),
             self._ptr(h_energy, torch.float64, n_blocks * self.W * 4, "cpu"),
             self._ptr(h_acc, torch.float64, n_blocks * self.W, "cpu") if h_acc is not None else None,
+            int(xyz_every),
+            self._ptr(h_xyz, torch.float64, n_xyz * self.W * 3 * self.N, "cpu") if h_xyz is not None else None,
             self._ptr(h_done, torch.int32, n_blocks, "cpu") if h_done is not None else None))
+
+    def sweep_writeouts(self, n_sweeps: int, steps, every: int, xyz_out, n_acc_out, flags):
+        """qmc_sweep_writeouts: ONE launch of n_sweeps sweeps whose thread blocks write coordinates / accepted-move
+        counts out every `every` sweeps and raise flags[k][w].  The tensors are device tensors, or pinned host tensors
+        (mapped into the device address space by CUDA's unified addressing), float64 / int64 / int32."""
+        torch = self._torch
+        n_out = n_sweeps // every
+        for t_, dt, n in ((xyz_out, torch.float64, n_out * self.W * 3 * self.N), (n_acc_out, torch.int64, n_out * self.W),
+                          (flags, torch.int32, n_out * self.W)):
+            if t_ is not None:
+                assert t_.dtype == dt and t_.is_contiguous() and t_.numel() >= n and (t_.is_cuda or t_.is_pinned())
+        self._check(self._lib.qmc_sweep_writeouts(
+            self._ctx, int(n_sweeps), self._steps(steps), int(every), C.c_void_p(xyz_out.data_ptr()),
+            C.c_void_p(n_acc_out.data_ptr()) if n_acc_out is not None else None, C.c_void_p(flags.data_ptr())))
 
     def wait(self):
         self._check(self._lib.qmc_wait(self._ctx))

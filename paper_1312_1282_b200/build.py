@@ -14,18 +14,21 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqmc_b200.so")
-SOURCES = ["qmc_api.cu", "qmc_sweep_plan.cu", "qmc_sweep_f32.cu", "qmc_sweep_f64.cu", "qmc_energy.cu", "qmc_energy_f32.cu", "qmc_energy_f32s.cu", "qmc_energy_f64.cu", "qmc_observables.cu"]
-HEADERS = ["qmc_device.cuh", "qmc_internal.h", "qmc_sweep_impl.cuh", "qmc_f32c.cuh", "qmc_energy_f32_pair.cuh", os.path.join("..", "..", "include", "qmc.h")]
+PROBE_LIB = os.path.join(HERE, "libqmc_probe_b200.so")      # measurement tool (include/qmc_probe.h), not the product
+PROBE_SRC = os.path.join(HERE, "probe", "qmc_probe.cu")
+SOURCES = ["qmc_api.cu", "qmc_sweep_plan.cu", "qmc_sweep_f32.cu", "qmc_sweep_f64.cu", "qmc_sweep_tile_f32.cu", "qmc_energy.cu",
+           "qmc_energy_f32.cu", "qmc_energy_f32s.cu", "qmc_energy_f64.cu", "qmc_observables.cu"]
+HEADERS = ["qmc_device.cuh", "qmc_internal.h", "qmc_sweep_impl.cuh", "qmc_sweep_tile.cuh", "qmc_f32c.cuh", "qmc_energy_f32_pair.cuh", os.path.join("..", "..", "include", "qmc.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 
 
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(PROBE_LIB):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    t = min(os.path.getmtime(LIB), os.path.getmtime(PROBE_LIB))
+    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__), PROBE_SRC]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
@@ -49,7 +52,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
         objs = list(ex.map(compile_one, SOURCES))
-    subprocess.check_call([NVCC, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
+    subprocess.check_call([NVCC, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a", "-ldl"])
+    subprocess.check_call([NVCC, *FLAGS, "-shared", "-o", PROBE_LIB, PROBE_SRC])
     return LIB
 
 

@@ -5,9 +5,18 @@
 #include <cstring>
 #include <new>
 
+#include <nvtx3/nvToolsExt.h>          // header-only NVTX v3: ranges around the hot launches
+
 #include "qmc_internal.h"
 
 using namespace qmc;
+
+namespace {
+struct NvtxRange {                      // no-op unless a profiler is attached
+    explicit NvtxRange(const char *name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
+}  // namespace
 
 static char g_create_err[512] = "no error";
 
@@ -50,8 +59,8 @@ template <typename Real>
 __global__ void init_kernel(StateView sv, uint2 key, double jitter)
 {
     const int N = sv.N, ld = sv.ld;
-    const int w = blockIdx.y;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int w = blockIdx.x;
+    const int i = blockIdx.y * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const GroupDev g = sv.groups[sv.group_of[w]];
     const long long k = g.k_lat, M = 4 * k * k * k;
@@ -79,8 +88,8 @@ template <typename Real>
 __global__ void set_positions_kernel(StateView sv, const double *__restrict__ xyz)
 {
     const int N = sv.N, ld = sv.ld;
-    const int w = blockIdx.y;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int w = blockIdx.x;
+    const int i = blockIdx.y * blockDim.x + threadIdx.x;
     if (i >= ld) return;
     Real *pos = reinterpret_cast<Real *>(sv.pos) + (size_t)w * 3 * ld;
     const double *src = xyz + (size_t)w * 3 * N;
@@ -102,8 +111,8 @@ template <typename Real>
 __global__ void get_positions_kernel(StateView sv, double *__restrict__ xyz)
 {
     const int N = sv.N, ld = sv.ld;
-    const int w = blockIdx.y;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int w = blockIdx.x;
+    const int i = blockIdx.y * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const Real *pos = reinterpret_cast<const Real *>(sv.pos) + (size_t)w * 3 * ld;
     double *dst = xyz + (size_t)w * 3 * N;
@@ -113,8 +122,8 @@ __global__ void get_positions_kernel(StateView sv, double *__restrict__ xyz)
 
 __global__ void get_pair_sums_kernel(StateView sv, double *__restrict__ S)
 {
-    const int w = blockIdx.y;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int w = blockIdx.x;
+    const int i = blockIdx.y * blockDim.x + threadIdx.x;
     // the state holds raw sums of t = y^5 + z^5 - sh; u = c1 t (qmc_sweep_impl.cuh)
     if (i < sv.N) S[(size_t)w * sv.N + i] = sv.groups[sv.group_of[w]].c1 * sv.S[(size_t)w * sv.ld + i];
 }
@@ -137,7 +146,8 @@ __global__ void zero_state_kernel(StateView sv, size_t pos_bytes)
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < (size_t)sv.W; i += (size_t)gridDim.x * blockDim.x) sv.n_acc[i] = 0ull;
 }
 
-static dim3 grid_wn(const qmc_ctx *c, int n) { return dim3((unsigned)((n + 127) / 128), (unsigned)c->W); }
+// walkers on gridDim.x (limit 2^31 - 1), particle tiles of 128 on gridDim.y
+static dim3 grid_wn(const qmc_ctx *c, int n) { return dim3((unsigned)c->W, (unsigned)((n + 127) / 128)); }
 
 cudaError_t launch_init(qmc_ctx *c)
 {
@@ -166,27 +176,6 @@ cudaError_t launch_acceptance(qmc_ctx *c, double *d_out)
     c->launches += 1;
     acceptance_kernel<<<(c->W + 127) / 128, 128, 0, c->stream>>>(c->sv, (double)(c->t - c->t_acc0) * (double)c->p.N, d_out);
     return cudaGetLastError();
-}
-
-// ------------------------------------------------------------------------------------------
-// FP pipe peak: 8 independent FMA chains per thread, 2048 threads per SM, no memory traffic.
-// ------------------------------------------------------------------------------------------
-template <typename Real>
-__global__ void __launch_bounds__(256) fma_peak_kernel(Real *sink, int iters, Real a, Real b)
-{
-    Real v[8];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) v[k] = (Real)(threadIdx.x + k);
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int rep = 0; rep < 8; ++rep)
-#pragma unroll
-            for (int k = 0; k < 8; ++k) v[k] = fma(v[k], a, b);
-    }
-    Real s = 0;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) s += v[k];
-    if (s == (Real)123456789) sink[0] = s;      // never true; keeps the chains alive
 }
 
 }  // namespace qmc
@@ -352,6 +341,7 @@ extern "C" int qmc_destroy(qmc_ctx *c)
     if (c->d_scratch) cudaFree(c->d_scratch);
     if (c->out_stream) cudaStreamSynchronize(c->out_stream);
     if (c->d_block) cudaFree(c->d_block);
+    if (c->d_block_xyz) cudaFree(c->d_block_xyz);
     for (int k = 0; k < 2; ++k) {
         if (c->ev_ready[k]) cudaEventDestroy(c->ev_ready[k]);
         if (c->ev_copied[k]) cudaEventDestroy(c->ev_copied[k]);
@@ -412,16 +402,35 @@ extern "C" int qmc_sweep(qmc_ctx *c, int32_t n_sweeps, const double *steps)
     }
     if (changed)   // stream-ordered update of the small constant table (host mirror is ours, pageable copy is synchronous to the host)
         QMC_CUDA(c, cudaMemcpyAsync(c->d_groups, c->groups.data(), sizeof(GroupDev) * c->p.n_groups, cudaMemcpyHostToDevice, c->stream));
-    QMC_CUDA(c, launch_sweep(c, n_sweeps));
+    {
+        NvtxRange r("qmc_sweep");
+        QMC_CUDA(c, launch_sweep(c, n_sweeps));
+    }
     c->t += (uint32_t)n_sweeps;
     if (c->trace.dec) c->trace.offset += (long long)n_sweeps * c->p.N;
     return QMC_OK;
+}
+
+extern "C" int qmc_sweep_writeouts(qmc_ctx *c, int32_t n_sweeps, const double *steps, int32_t every,
+                                   double *xyz_out, uint64_t *n_acc_out, int32_t *flags)
+{
+    if (!c) return QMC_E_ARG;
+    if (every < 1 || !xyz_out || !flags) QMC_FAIL(c, QMC_E_ARG, "every >= 1, xyz_out and flags are required");
+    c->wo.xyz = xyz_out;
+    c->wo.n_acc = reinterpret_cast<unsigned long long *>(n_acc_out);
+    c->wo.flag = flags;
+    c->wo.every = every;
+    c->wo.n_out = n_sweeps / every;
+    const int rc = qmc_sweep(c, n_sweeps, steps);
+    c->wo = WriteoutView{};
+    return rc;
 }
 
 extern "C" int qmc_local_energy(qmc_ctx *c, double *d_out)
 {
     if (!c || !d_out) return QMC_E_ARG;
     if (!c->have_state) QMC_FAIL(c, QMC_E_STATE, "qmc_local_energy before qmc_init_walkers / qmc_set_positions");
+    NvtxRange r("qmc_local_energy");
     QMC_CUDA(c, launch_energy(c, d_out, true));
     return QMC_OK;
 }
@@ -531,34 +540,56 @@ extern "C" int qmc_step_host(qmc_ctx *c, const double *h_xyz_in, int32_t n_sweep
 static void CUDART_CB raise_flag(void *flag) { *reinterpret_cast<volatile int32_t *>(flag) = 1; }
 
 extern "C" int qmc_run_blocks_host(qmc_ctx *c, int32_t n_blocks, int32_t sweeps_per_block, const double *steps,
-                                   double *h_energy, double *h_acc, int32_t *h_done)
+                                   double *h_energy, double *h_acc, int32_t xyz_every, double *h_xyz, int32_t *h_done)
 {
     if (!c || !h_energy) return QMC_E_ARG;
     if (!c->have_state) QMC_FAIL(c, QMC_E_STATE, "qmc_run_blocks_host before qmc_init_walkers / qmc_set_positions");
     if (n_blocks < 0 || sweeps_per_block < 1) QMC_FAIL(c, QMC_E_ARG, "n_blocks >= 0 and sweeps_per_block >= 1 required");
-    const size_t W = (size_t)c->W;
-    if (!c->out_stream) {
-        QMC_CUDA(c, cudaStreamCreateWithFlags(&c->out_stream, cudaStreamNonBlocking));
-        QMC_CUDA(c, cudaMalloc(&c->d_block, sizeof(double) * 2 * W * 5));
-        for (int k = 0; k < 2; ++k) {
-            QMC_CUDA(c, cudaEventCreateWithFlags(&c->ev_ready[k], cudaEventDisableTiming));
-            QMC_CUDA(c, cudaEventCreateWithFlags(&c->ev_copied[k], cudaEventDisableTiming));
+    if (h_xyz && xyz_every < 1) QMC_FAIL(c, QMC_E_ARG, "xyz_every >= 1 required with h_xyz");
+    const size_t W = (size_t)c->W, N = (size_t)c->p.N;
+    // first use: write-out stream, double-buffered results, events.  Everything or nothing: a failure half way
+    // leaves no half-initialised state behind for the next call.
+    if (!c->blocks_ready) {
+        auto undo = [&]() {
+            if (c->out_stream) { cudaStreamDestroy(c->out_stream); c->out_stream = nullptr; }
+            if (c->d_block) { cudaFree(c->d_block); c->d_block = nullptr; }
+            for (int k = 0; k < 2; ++k) {
+                if (c->ev_ready[k]) { cudaEventDestroy(c->ev_ready[k]); c->ev_ready[k] = nullptr; }
+                if (c->ev_copied[k]) { cudaEventDestroy(c->ev_copied[k]); c->ev_copied[k] = nullptr; }
+            }
+        };
+        cudaError_t e = cudaStreamCreateWithFlags(&c->out_stream, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaMalloc(&c->d_block, sizeof(double) * 2 * W * 5);
+        for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+            e = cudaEventCreateWithFlags(&c->ev_ready[k], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_copied[k], cudaEventDisableTiming);
         }
+        if (e != cudaSuccess) { undo(); QMC_FAIL(c, QMC_E_CUDA, "qmc_run_blocks_host set-up: %s", cudaGetErrorString(e)); }
+        c->blocks_ready = true;
     }
+    if (h_xyz && !c->d_block_xyz) QMC_CUDA(c, cudaMalloc(&c->d_block_xyz, sizeof(double) * 2 * W * 3 * N));
     for (int32_t b = 0; b < n_blocks; ++b) {
         const int k = b & 1;
         double *d_e = c->d_block + (size_t)k * W * 5, *d_a = d_e + 4 * W;
         int rc = qmc_sweep(c, sweeps_per_block, steps);
         if (rc != QMC_OK) return rc;
-        if (b >= 2) QMC_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copied[k], 0));   // buffer k is free again
+        // buffer k is free again once its last copy has finished -- also the copy of an EARLIER call (waiting on an
+        // event that was never recorded is a no-op)
+        QMC_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copied[k], 0));
         if ((rc = qmc_local_energy(c, d_e)) != QMC_OK) return rc;
         if ((rc = qmc_acceptance(c, d_a)) != QMC_OK) return rc;
+        const bool with_xyz = h_xyz && ((b + 1) % xyz_every == 0);
+        double *d_x = c->d_block_xyz ? c->d_block_xyz + (size_t)k * W * 3 * N : nullptr;
+        if (with_xyz && (rc = qmc_get_positions(c, d_x)) != QMC_OK) return rc;
         QMC_CUDA(c, cudaEventRecord(c->ev_ready[k], c->stream));
         // write-out while the next block computes (the paper's asynchronous writeouts, l.175, l.323)
         QMC_CUDA(c, cudaStreamWaitEvent(c->out_stream, c->ev_ready[k], 0));
         QMC_CUDA(c, cudaMemcpyAsync(h_energy + (size_t)b * W * 4, d_e, sizeof(double) * 4 * W, cudaMemcpyDeviceToHost, c->out_stream));
         if (h_acc)
             QMC_CUDA(c, cudaMemcpyAsync(h_acc + (size_t)b * W, d_a, sizeof(double) * W, cudaMemcpyDeviceToHost, c->out_stream));
+        if (with_xyz)
+            QMC_CUDA(c, cudaMemcpyAsync(h_xyz + (size_t)((b + 1) / xyz_every - 1) * W * 3 * N, d_x, sizeof(double) * W * 3 * N,
+                                        cudaMemcpyDeviceToHost, c->out_stream));
         QMC_CUDA(c, cudaEventRecord(c->ev_copied[k], c->out_stream));
         if (h_done) QMC_CUDA(c, cudaLaunchHostFunc(c->out_stream, raise_flag, h_done + b));
     }
@@ -584,84 +615,23 @@ extern "C" int qmc_info(const qmc_ctx *c, qmc_info_t *out)
     out->sm_count = c->sm_count;
     out->t = c->t;
     out->kernel_launches = c->launches;
+    out->sweep_vector = c->sweep_plan.V; out->sweep_pending = c->sweep_plan.P; out->sweep_tile = c->sweep_plan.K;
+    out->energy_variant = c->energy_plan.variant;
+    out->sweep_cluster = c->sweep_plan.cluster;
     return QMC_OK;
 }
 
-// Instruction-rate probes behind qmc_pipe_peak kinds 2..5: 8 independent chains per thread of one
-// instruction kind (inline PTX, so that the kind in SASS is the one named), no memory traffic.
-namespace qmc {
-template <int KIND>
-__global__ void __launch_bounds__(256) rate_probe_kernel(float *sink, int iters, float a, float b)
+extern "C" int qmc_set_tuning(const char *key, int32_t value)
 {
-    float v[8];
-    unsigned long long p[8], pa, pb;
-    double d[8];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-        v[k] = a + (float)(threadIdx.x + k);
-        asm("mov.b64 %0, {%1, %2};" : "=l"(p[k]) : "f"(v[k]), "f"(v[k] + 0.5f));
-        d[k] = (double)v[k];
-    }
-    asm("mov.b64 %0, {%1, %1};" : "=l"(pa) : "f"(a));
-    asm("mov.b64 %0, {%1, %1};" : "=l"(pb) : "f"(b));
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int rep = 0; rep < 8; ++rep)
-#pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                if (KIND == 2) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(p[k]) : "l"(pa), "l"(pb));
-                if (KIND == 3) asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(v[k]));
-                if (KIND == 4) asm volatile("{.reg .s32 t; mov.b32 t, %0; cvt.rn.f32.s32 %0, t;}" : "+f"(v[k]));
-                if (KIND == 5) asm volatile("{.reg .f32 t; cvt.rn.f32.f64 t, %0; cvt.f64.f32 %0, t;}" : "+d"(d[k]));
-            }
-    }
-    float s = 0;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-        float lo, hi;
-        asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(p[k]));
-        s += v[k] + lo + hi + (float)d[k];
-    }
-    if (s == 123456789.0f) sink[0] = s;         // never true; keeps the chains alive
-}
-}  // namespace qmc
-
-extern "C" int qmc_pipe_peak(int32_t which, void *cuda_stream, double *h_fma_per_s)
-{
-    if (!h_fma_per_s || which < 0 || which > 5) return QMC_E_ARG;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
-        snprintf(g_create_err, 512, "no CUDA device");
-        return QMC_E_CUDA;
-    }
-    void *sink = nullptr;
-    if (cudaMalloc(&sink, 64) != cudaSuccess) return QMC_E_CUDA;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    const int iters = which == 1 ? 8000 : (which == 0 || which == 2 || which == 4 ? 4000 : 1000);
-    const int grid = sms * 8, block = 256;
-    float best_ms = 1e30f;
-    for (int rep = 0; rep < 4; ++rep) {
-        cudaEventRecord(e0, st);
-        switch (which) {
-        case 0: fma_peak_kernel<double><<<grid, block, 0, st>>>((double *)sink, iters, 0.999999, 1e-7); break;
-        case 1: fma_peak_kernel<float><<<grid, block, 0, st>>>((float *)sink, iters, 0.999999f, 1e-7f); break;
-        case 2: rate_probe_kernel<2><<<grid, block, 0, st>>>((float *)sink, iters, 0.999999f, 1e-7f); break;
-        case 3: rate_probe_kernel<3><<<grid, block, 0, st>>>((float *)sink, iters, 0.999999f, 1e-7f); break;
-        case 4: rate_probe_kernel<4><<<grid, block, 0, st>>>((float *)sink, iters, 0.999999f, 1e-7f); break;
-        default: rate_probe_kernel<5><<<grid, block, 0, st>>>((float *)sink, iters, 0.999999f, 1e-7f); break;
-        }
-        cudaEventRecord(e1, st);
-        cudaEventSynchronize(e1);
-        float ms = 0;
-        cudaEventElapsedTime(&ms, e0, e1);
-        if (rep > 0 && ms < best_ms) best_ms = ms;
-    }
-    cudaError_t e = cudaGetLastError();
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
-    if (e != cudaSuccess) { snprintf(g_create_err, 512, "pipe peak kernel: %s", cudaGetErrorString(e)); return QMC_E_CUDA; }
-    const double per_iter = which == 5 ? 128.0 : 64.0;          // kind 5 issues two conversions per chain step
-    *h_fma_per_s = (double)grid * block * (double)iters * per_iter / (best_ms * 1e-3);
-    return QMC_OK;
+    Tuning &t = g_tuning;
+    if (!key) { t = Tuning{}; return QMC_OK; }
+    struct { const char *name; int *field; } tab[] = {
+        {"sweep_threads", &t.sweep_threads}, {"sweep_per_thread", &t.sweep_per_thread}, {"sweep_vector", &t.sweep_vector},
+        {"sweep_pending", &t.sweep_pending}, {"sweep_tile", &t.sweep_tile}, {"sweep_cluster", &t.sweep_cluster},
+        {"energy_threads", &t.energy_threads}, {"energy_ordered", &t.energy_ordered},
+    };
+    for (auto &e : tab)
+        if (strcmp(key, e.name) == 0) { *e.field = value; return QMC_OK; }
+    snprintf(g_create_err, 512, "qmc_set_tuning: unknown key '%s'", key);
+    return QMC_E_ARG;
 }

@@ -182,43 +182,6 @@ struct PairConst {
     }
 };
 
-// Squared minimum-image distance between a and b.
-template <typename Real>
-__device__ __forceinline__ Real min_image_r2(Real ax, Real ay, Real az, Real bx, Real by, Real bz,
-                                             const PairConst<Real> &P)
-{
-    const Real mx = P.h - rabs<Real>(P.h - rabs<Real>(ax - bx));
-    const Real my = P.h - rabs<Real>(P.h - rabs<Real>(ay - by));
-    const Real mz = P.h - rabs<Real>(P.h - rabs<Real>(az - bz));
-    return fma(mz, mz, fma(my, my, mx * mx));
-}
-
-// u(r) from r^2 without the cutoff select (the caller selects on r^2 < h^2 together with its other
-// conditions).  NaN in -> NaN out, nothing traps.
-template <typename Real>
-__device__ __forceinline__ Real pair_u_raw(Real r2, const PairConst<Real> &P)
-{
-    const Real y = rsqrt_pos(r2);
-    const Real r = r2 * y;
-    const Real z = rcp_pos(P.L - r);
-    const Real y2 = y * y, z2 = z * z;
-    const Real y5 = y2 * y2 * y, z5 = z2 * z2 * z;
-    return fma(P.c1, y5 + z5, P.c0);
-}
-
-// u(r) from r^2 (> 0); 0 at and beyond the cutoff (strict '<', R2).
-template <typename Real>
-__device__ __forceinline__ Real pair_u(Real r2, const PairConst<Real> &P)
-{
-    const Real y = rsqrt_pos(r2);
-    const Real r = r2 * y;
-    const Real z = rcp_pos(P.L - r);
-    const Real y2 = y * y, z2 = z * z;
-    const Real y5 = y2 * y2 * y, z5 = z2 * z2 * z;
-    const Real u = fma(P.c1, y5 + z5, P.c0);
-    return r2 < P.h2 ? u : (Real)0;
-}
-
 // ---------------------------------------------------------------------------------------------
 // Warp / block sums.  The xor butterfly leaves the bitwise-identical total in every lane
 // (IEEE addition commutes), so every thread can take the same decision without a broadcast.

@@ -10,24 +10,16 @@
 //   Lambda_i = sum_{j != i} [u'' + 2 u'/r]                     =  -b^5 (10 y^7 + 15 z^7 + 5 z^6 y)
 //   V        = sum_{i<j, r<h} V_Aziz(r_ij)                 (HFD-B(HE), truncated at h, R3)
 //   T_PB = -Dk sum_i (Lambda_i + |G_i|^2),  T_JF = -Dk/2 sum_i Lambda_i,  E_PB = V + T_PB   (R14)
-// with y = 1/r, z = 1/(L-r).  In FP32C the per-pair terms are fp32; they are summed in fp32 over
-// blocks of kFlush consecutive j and then added to fp64 accumulators (R20).
+// with y = 1/r, z = 1/(L-r).  This ordered-pair kernel is the FP64 fallback for N whose per-particle accumulators do
+// not fit the unordered-pair kernel of qmc_energy_f64.cu (N > ~4100) and the dispatcher of all energy kernels.
 #include "qmc_internal.h"
 
 namespace qmc {
 
 constexpr int kFlush = 16;
 
-// Constants of the energy pass in the arithmetic type of the mode.
-//
-// FP64: the potential as DESIGN.md §2 writes it.
-// FP32C: every constant that multiplies into the steep repulsive exponential or the dispersion sum is
-// either folded (in fp64, on load) into ONE rounded coefficient or carried as a hi + lo pair, so that no
-// fp32 rounding of a CONSTANT adds a systematic relative error to every pair (the box-unit value of r_m
-// is an arbitrary real number; its fp32 rounding alone would shift the exponent argument by ~6e-7):
-//   rep  = eps A exp(a1 r + a2 r^2),  a1 = -alpha / r_m,  a2 = beta / r_m^2   (hi + lo)
-//   disp = w^3 (k6 + w (k8 + w k10)),  w = fl(r_m^2) y^2,  k_n = eps c_n (r_m^2 / fl(r_m^2))^(n/2)
-//   F    = exp(-(D r_m y - 1)^2)                                                  (D r_m hi + lo)
+// Constants of the potential as DESIGN.md §2 writes it (this file serves FP64 only; the FP32C kernels are
+// qmc_energy_f32.cu and qmc_energy_f32s.cu).
 template <typename Real> struct EnergyConst;
 
 template <> struct EnergyConst<double> {
@@ -37,29 +29,6 @@ template <> struct EnergyConst<double> {
         b5 = g.b5; eps = a.eps; inv_rm = a.inv_rm; rm2 = a.rm2; A = a.A;
         alpha = a.alpha; beta = a.beta; c6 = a.c6; c8 = a.c8; c10 = a.c10;
         D = a.D; Drm = a.Drm;
-    }
-};
-
-__device__ __forceinline__ void split_hi_lo(double v, float &hi, float &lo)
-{
-    hi = __double2float_rn(v);
-    lo = __double2float_rn(v - (double)hi);
-}
-
-template <> struct EnergyConst<float> {
-    float b5, a1h, a1l, a2h, a2l, epsA, rm2, k6, k8, k10, Drm, Drml;
-    __device__ __forceinline__ void load(const GroupDev &g, const AzizDev &a)
-    {
-        b5 = (float)g.b5;
-        split_hi_lo(-a.alpha * a.inv_rm, a1h, a1l);
-        split_hi_lo(a.beta * a.inv_rm * a.inv_rm, a2h, a2l);
-        epsA = (float)(a.eps * a.A);
-        rm2 = (float)a.rm2;
-        const double q = a.rm2 / (double)rm2;             // 1 + rounding error of fl(r_m^2)
-        k6 = (float)(a.eps * a.c6 * q * q * q);
-        k8 = (float)(a.eps * a.c8 * q * q * q * q);
-        k10 = (float)(a.eps * a.c10 * q * q * q * q * q);
-        split_hi_lo(a.Drm, Drm, Drml);
     }
 };
 
@@ -84,30 +53,6 @@ __device__ __forceinline__ double aziz_pair(double, double r, double y, const En
     }
     const double rep = E.A * exp(x * fma(E.beta, x, -E.alpha));
     return E.eps * (rep - F * disp);
-}
-
-// FP32C: y is first refined by one Newton step (the hardware rsqrt seed is good to ~2^-22, and the
-// repulsive exponential amplifies a relative error of r ~11x); the exponent argument is carried as
-// hi + lo, exp(hi + lo) = exp(hi) (1 + lo).
-__device__ __forceinline__ float aziz_pair(float r2, float, float y0, const EnergyConst<float> &E)
-{
-    const float e = fmaf(-r2 * y0, y0, 1.0f);
-    const float y = fmaf(0.5f * y0, e, y0);
-    const float r = r2 * y;
-    const float w = E.rm2 * y * y;
-    const float disp = w * w * w * fmaf(w, fmaf(w, E.k10, E.k8), E.k6);
-    float F = 1.0f;
-    if (r < E.Drm) {
-        const float t = fmaf(E.Drml, y, fmaf(E.Drm, y, -1.0f));
-        F = expf(-t * t);
-    }
-    const float t1 = fmaf(E.a2h, r, E.a1h);
-    const float ah = r * t1;
-    float al = fmaf(r, t1, -ah);                                // exact residual of the product
-    al = fmaf(r, fmaf(E.a2l, r, E.a1l), al);
-    const float ex = E.epsA * expf(ah);
-    const float rep = fmaf(ex, al, ex);
-    return rep - F * disp;
 }
 
 template <typename Real, int T, bool kEnergy>
@@ -257,17 +202,17 @@ bool plan_energy(qmc_ctx *c, EnergyPlan *out)
 {
     out->variant = 0;
     if (c->p.mode != QMC_FP64) {
-        if (!getenv("QMC_ENERGY_ORDERED") && plan_energy_f32s(c, out)) return true;
+        if (!g_tuning.energy_ordered && plan_energy_f32s(c, out)) return true;
         out->variant = 0;
         return plan_energy_f32(c, out);
     }
-    if (!getenv("QMC_ENERGY_ORDERED") && plan_energy_f64(c, out)) return true;
+    if (!g_tuning.energy_ordered && plan_energy_f64(c, out)) return true;
     out->variant = 0;
     const int N = c->p.N;
     int T = 32;
     while (T < N && T < 256) T *= 2;
-    if (const char *env = getenv("QMC_ENERGY_THREADS")) {
-        const int v = atoi(env);
+    if (g_tuning.energy_threads > 0) {
+        const int v = g_tuning.energy_threads;
         if (v >= 32 && v <= 1024 && (v & (v - 1)) == 0) T = v;
     }
     out->threads = T;

@@ -239,15 +239,15 @@ cudaError_t launch_energy_f32(qmc_ctx *c, double *d_out, bool energy)
     return cudaErrorInvalidValue;
 }
 
-// One warp per 32 particles up to 8 warps; QMC_ENERGY_THREADS overrides (tuning experiments).
+// One warp per 32 particles up to 8 warps; qmc_set_tuning("energy_threads") overrides (tuning experiments).
 bool plan_energy_f32(qmc_ctx *c, EnergyPlan *out)
 {
     const int N = c->p.N;
     int T = 32;
     while (T < N && T < 256) T *= 2;
     if (smem_bytes32(N) > 113 * 1024) T = 512;      // one CTA per SM (N = 10000): fill it with 16 warps
-    if (const char *env = getenv("QMC_ENERGY_THREADS")) {
-        const int v = atoi(env);
+    if (g_tuning.energy_threads > 0) {
+        const int v = g_tuning.energy_threads;
         if (v >= 32 && v <= 512 && (v & (v - 1)) == 0) T = v;
     }
     out->threads = T;

@@ -15,7 +15,7 @@
 // their constants removed in fp64.
 //
 // R20: per-pair terms are fp32; at most 16 of them are summed in fp32 (two packed lanes of 8) before they are
-// added to an fp64 accumulator (registers for i, shared-memory atomics for j and at the end of a block row).
+// added to an fp64 accumulator (per-lane accumulators for i, shared memory for j; fixed order, reproducible to the bit).
 #include "qmc_energy_f32_pair.cuh"
 
 namespace qmc {
@@ -23,6 +23,8 @@ namespace qmc {
 namespace {
 
 using namespace e32;
+
+constexpr int kMaxOwn32 = 20;                        // i-blocks one warp can own (planner: ceil(nblk / nwarps) <= kMaxOwn32)
 
 __device__ __forceinline__ float shfl_f(float v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 
@@ -92,7 +94,7 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
     const int nblk = (N + 31) >> 5, NP = nblk << 5;
 
     double  *red = reinterpret_cast<double *>(smem_raw);              // [3][32]
-    int     *ctr = reinterpret_cast<int *>(red + 96);                 // work counter; red[97]: opaque zero
+                                                                      // red[97]: opaque zero
     double  *ag  = red + 98;                                          // [4][NP]: G_x, G_y, G_z (2^32 box units), S
     int32_t *x   = reinterpret_cast<int32_t *>(ag + 4 * NP);          // [3][NP]
     int32_t *y = x + NP, *z = x + 2 * NP;
@@ -109,7 +111,7 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
         z[j] = in ? enc_coord(gpos[2 * ld + j]) : 0;
         ag[j] = 0.0; ag[NP + j] = 0.0; ag[2 * NP + j] = 0.0; ag[3 * NP + j] = 0.0;
     }
-    if (tid == 0) { *ctr = 0; *reinterpret_cast<int32_t *>(red + 97) = 0; }
+    if (tid == 0) *reinterpret_cast<int32_t *>(red + 97) = 0;
     __syncthreads();
     const int32_t zero = opaque_zero(reinterpret_cast<int32_t *>(red + 97));
 
@@ -121,21 +123,28 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
         KV = va;
     }
 
+    // Schedule as in qmc_energy_f64.cu (deterministic): warp v owns the i-blocks A = v, v + nwarps, ...;
+    // all warps step through the ring offsets k together (one barrier per offset), so within one offset the j-blocks
+    // B = A + k of different warps are different and the j-side sums are added to shared memory by plain
+    // read-modify-writes in the order of k; the i-side sums wait in local accumulators until the last offset.
     const int K = (nblk - 1) >> 1;
     const bool even = (nblk & 1) == 0, ragged = (N & 31) != 0;
     double tLam = 0.0, tV = 0.0;
     long long slots = 0, inside = 0;
-    for (;;) {
-        int A = 0;
-        if (lane == 0) A = atomicAdd(ctr, 1);
-        A = __shfl_sync(0xffffffffu, A, 0);
-        if (A >= nblk) break;
-        const int i = (A << 5) + lane;
-        const bool vi = i < N;
-        const int32_t xi = x[i], yi = y[i], zi = z[i];
-        double gxi = 0.0, gyi = 0.0, gzi = 0.0, si = 0.0;
-        const int kmax = K + ((even && A < (nblk >> 1)) ? 1 : 0);
-        for (int k = 0; k <= kmax; ++k) {
+    double own[kMaxOwn32][4];                                         // G_x, G_y, G_z, S of this lane's particle in each own block
+#pragma unroll 1
+    for (int a = 0; a < kMaxOwn32; ++a) { own[a][0] = 0.0; own[a][1] = 0.0; own[a][2] = 0.0; own[a][3] = 0.0; }
+    const int kend = K + (even ? 1 : 0);
+#pragma unroll 1
+    for (int k = 0; k <= kend; ++k) {
+        int a = 0;
+#pragma unroll 1
+        for (int A = warp; A < nblk; A += nwarps, ++a) {
+            if (k > K && A >= (nblk >> 1)) break;                    // even n: the offset n/2 once per block pair
+            const int i = (A << 5) + lane;
+            const bool vi = i < N;
+            const int32_t xi = x[i], yi = y[i], zi = z[i];
+            double gxi = 0.0, gyi = 0.0, gzi = 0.0, si = 0.0;
             int B = A + k;
             if (B >= nblk) B -= nblk;
             const int jb = B << 5;
@@ -161,20 +170,26 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
                 }
             }
             if (jb + lane < N) {
-                atomicAdd(&ag[3 * NP + jb + lane], sj);
+                ag[3 * NP + jb + lane] += sj;
                 if (kEnergy) {
-                    atomicAdd(&ag[jb + lane], -gxj);
-                    atomicAdd(&ag[NP + jb + lane], -gyj);
-                    atomicAdd(&ag[2 * NP + jb + lane], -gzj);
+                    ag[jb + lane] -= gxj;
+                    ag[NP + jb + lane] -= gyj;
+                    ag[2 * NP + jb + lane] -= gzj;
                 }
             }
+            own[a][3] += si;
+            if (kEnergy) { own[a][0] += gxi; own[a][1] += gyi; own[a][2] += gzi; }
         }
-        if (vi) {
-            atomicAdd(&ag[3 * NP + i], si);
-            if (kEnergy) {
-                atomicAdd(&ag[i], gxi);
-                atomicAdd(&ag[NP + i], gyi);
-                atomicAdd(&ag[2 * NP + i], gzi);
+        __syncthreads();
+    }
+    {
+        int a = 0;
+#pragma unroll 1
+        for (int A = warp; A < nblk; A += nwarps, ++a) {
+            const int i = (A << 5) + lane;
+            if (i < N) {
+                ag[3 * NP + i] += own[a][3];
+                if (kEnergy) { ag[i] += own[a][0]; ag[NP + i] += own[a][1]; ag[2 * NP + i] += own[a][2]; }
             }
         }
     }
@@ -256,7 +271,7 @@ cudaError_t launch_energy_f32s(qmc_ctx *c, double *d_out, bool energy)
 }
 
 // false: the per-particle fp64 accumulators do not leave room for two CTAs per SM (N > ~2500) -- the caller
-// keeps the ordered-pair kernel.  QMC_ENERGY_THREADS overrides the thread count (tuning experiments).
+// keeps the ordered-pair kernel.  qmc_set_tuning("energy_threads") overrides the thread count (tuning experiments).
 bool plan_energy_f32s(qmc_ctx *c, EnergyPlan *out)
 {
     const int N = c->p.N;
@@ -264,10 +279,13 @@ bool plan_energy_f32s(qmc_ctx *c, EnergyPlan *out)
     if (smem > 113 * 1024) return false;
     int T = 32;
     while (2 * T < N && T < 256) T *= 2;
-    if (const char *env = getenv("QMC_ENERGY_THREADS")) {
-        const int v = atoi(env);
+    if (g_tuning.energy_threads > 0) {
+        const int v = g_tuning.energy_threads;
         if (v >= 32 && v <= 512 && (v & (v - 1)) == 0) T = v;
     }
+    const int nblk = (N + 31) >> 5;
+    while ((nblk + (T >> 5) - 1) / (T >> 5) > kMaxOwn32 && T < 512) T *= 2;     // own-block accumulators per warp
+    if ((nblk + (T >> 5) - 1) / (T >> 5) > kMaxOwn32) return false;
     out->threads = T;
     out->smem_bytes = smem;
     out->variant = 2;

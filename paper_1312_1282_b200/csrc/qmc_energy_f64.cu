@@ -8,7 +8,8 @@
 // (i_l, j_{(l+s) mod 32}).  The i-side sums stay in the lane's registers; the j-side terms travel by one
 // indexed shuffle to the lane that holds j.  Block pairs are visited along a ring, B = A + k mod n,
 // k = 1 .. (n-1)/2 (+ half of k = n/2 for even n), the diagonal block with steps 1..16: each pair once.
-// Per-block sums are merged with shared-memory atomics (a few per 1024 pairs).
+// Block ownership is static and the warps step through k together, so the per-block sums are merged by plain
+// shared-memory read-modify-writes in a fixed order: results are reproducible to the bit.
 //
 //   G_i      = sum_{j != i} u'(r_ij) d_ij / r_ij,     u'/r = 5/2 b^5 (y^7 - z^6 y)
 //   Lambda_i = sum_{j != i} [u'' + 2 u'/r]                 = -5 b^5 (2 y^7 + 3 z^7 + z^6 y)
@@ -30,6 +31,7 @@ namespace qmc {
 namespace {
 
 constexpr int kUnroll64 = QMC_E64_UNROLL;            // pair steps in flight per lane
+constexpr int kMaxOwn64 = 20;                        // i-blocks one warp can own (planner: ceil(nblk / nwarps) <= kMaxOwn64)
 
 struct Const64 {
     double L, h, h2, sh;
@@ -135,7 +137,6 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
     const int nblk = (N + 31) >> 5, NP = nblk << 5;
 
     double *red = reinterpret_cast<double *>(smem_raw);               // [3][32]
-    int    *ctr = reinterpret_cast<int *>(red + 96);                  // work counter (+ padding to 16 bytes)
     double *x   = red + 98;                                           // [3][NP]
     double *y = x + NP, *z = x + 2 * NP;
     double *ag = x + 3 * NP;                                          // [4][NP]: G_x, G_y, G_z, S (raw units)
@@ -152,25 +153,32 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
         z[j] = in ? gpos[2 * ld + j] : 0.0;
         ag[j] = 0.0; ag[NP + j] = 0.0; ag[2 * NP + j] = 0.0; ag[3 * NP + j] = 0.0;
     }
-    if (tid == 0) *ctr = 0;
     __syncthreads();
 
     const double kBig = 4.0 * C.L * C.L;                              // > any r^2: forces the clamp
 
+    // Schedule (deterministic: the same sums in the same order on every run): warp v owns the i-blocks
+    // A = v, v + nwarps, ...; all warps go through the ring offsets k = 0, 1, ... together, one barrier per offset.
+    // Within one offset the j-blocks B = A + k mod n of different A are different, so the j-side sums are added
+    // to shared memory by plain read-modify-writes of the one warp that holds them, in the order of k; the i-side
+    // sums of a warp's own blocks wait in (local-memory) accumulators and are added after the last offset.
     const int K = (nblk - 1) >> 1;                                    // full ring offsets
     const bool even = (nblk & 1) == 0;
     double tLam = 0.0, tV = 0.0;
-    for (;;) {
-        int A = 0;
-        if (lane == 0) A = atomicAdd(ctr, 1);
-        A = __shfl_sync(0xffffffffu, A, 0);
-        if (A >= nblk) break;
-        const int i = (A << 5) + lane;
-        const bool vi = i < N;
-        const double xi = x[i], yi = y[i], zi = z[i];
-        double gxi = 0.0, gyi = 0.0, gzi = 0.0, si = 0.0;
-        const int kmax = K + ((even && A < (nblk >> 1)) ? 1 : 0);
-        for (int k = 0; k <= kmax; ++k) {
+    double own[kMaxOwn64][4];                                         // G_x, G_y, G_z, S of this lane's particle in each own block
+#pragma unroll 1
+    for (int a = 0; a < kMaxOwn64; ++a) { own[a][0] = 0.0; own[a][1] = 0.0; own[a][2] = 0.0; own[a][3] = 0.0; }
+    const int kend = K + (even ? 1 : 0);
+#pragma unroll 1
+    for (int k = 0; k <= kend; ++k) {
+        int a = 0;
+#pragma unroll 1
+        for (int A = warp; A < nblk; A += nwarps, ++a) {
+            if (k > K && A >= (nblk >> 1)) break;                    // even n: the offset n/2 once per block pair
+            const int i = (A << 5) + lane;
+            const bool vi = i < N;
+            const double xi = x[i], yi = y[i], zi = z[i];
+            double gxi = 0.0, gyi = 0.0, gzi = 0.0, si = 0.0;
             int B = A + k;
             if (B >= nblk) B -= nblk;
             const int jb = B << 5;
@@ -200,20 +208,26 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
                 }
             }
             if (vj) {
-                atomicAdd(&ag[3 * NP + jb + lane], sj);
+                ag[3 * NP + jb + lane] += sj;
                 if (kEnergy) {
-                    atomicAdd(&ag[jb + lane], gxj);
-                    atomicAdd(&ag[NP + jb + lane], gyj);
-                    atomicAdd(&ag[2 * NP + jb + lane], gzj);
+                    ag[jb + lane] += gxj;
+                    ag[NP + jb + lane] += gyj;
+                    ag[2 * NP + jb + lane] += gzj;
                 }
             }
+            own[a][3] += si;
+            if (kEnergy) { own[a][0] += gxi; own[a][1] += gyi; own[a][2] += gzi; }
         }
-        if (vi) {
-            atomicAdd(&ag[3 * NP + i], si);
-            if (kEnergy) {
-                atomicAdd(&ag[i], gxi);
-                atomicAdd(&ag[NP + i], gyi);
-                atomicAdd(&ag[2 * NP + i], gzi);
+        __syncthreads();
+    }
+    {
+        int a = 0;
+#pragma unroll 1
+        for (int A = warp; A < nblk; A += nwarps, ++a) {
+            const int i = (A << 5) + lane;
+            if (i < N) {
+                ag[3 * NP + i] += own[a][3];
+                if (kEnergy) { ag[i] += own[a][0]; ag[NP + i] += own[a][1]; ag[2 * NP + i] += own[a][2]; }
             }
         }
     }
@@ -294,7 +308,7 @@ cudaError_t launch_energy_f64(qmc_ctx *c, double *d_out, bool energy)
 }
 
 // One warp per 64 particles (a block of 32 has about n/2 block pairs to go through), 1 to 8 warps;
-// QMC_ENERGY_THREADS overrides (tuning experiments).  false: N too large for the per-particle
+// qmc_set_tuning("energy_threads") overrides (tuning experiments).  false: N too large for the per-particle
 // accumulators in shared memory -- the caller falls back to the ordered-pair kernel of qmc_energy.cu.
 bool plan_energy_f64(qmc_ctx *c, EnergyPlan *out)
 {
@@ -303,10 +317,13 @@ bool plan_energy_f64(qmc_ctx *c, EnergyPlan *out)
     if (smem > 227 * 1024) return false;
     int T = 32;
     while (2 * T < N && T < 256) T *= 2;
-    if (const char *env = getenv("QMC_ENERGY_THREADS")) {
-        const int v = atoi(env);
+    if (g_tuning.energy_threads > 0) {
+        const int v = g_tuning.energy_threads;
         if (v >= 32 && v <= 512 && (v & (v - 1)) == 0) T = v;
     }
+    const int nblk = (N + 31) >> 5;
+    while ((nblk + (T >> 5) - 1) / (T >> 5) > kMaxOwn64 && T < 512) T *= 2;     // own-block accumulators per warp
+    if ((nblk + (T >> 5) - 1) / (T >> 5) > kMaxOwn64) return false;
     out->threads = T;
     out->smem_bytes = smem;
     out->variant = 1;

@@ -29,7 +29,24 @@ struct TraceView {
     long long capacity, offset;   // offset = moves already recorded per walker
 };
 
-struct SweepPlan  { int threads, J, V, smem_bytes, ctas_per_sm; const void *shape; };
+// In-kernel write-outs: every `every` sweeps the CTA writes
+// its walker's coordinates and accepted-move count to a buffer the host can read while the kernel runs (mapped
+// pinned host memory, or device memory) and then raises the walker's flag of that write-out (the paper's
+// sentinel values in write-combined memory, as an explicit flag array).
+struct WriteoutView {
+    double *xyz;                   // [n_out][W][3][N] Angstrom, or nullptr: no write-outs
+    unsigned long long *n_acc;     // [n_out][W] accepted moves since init / set_positions, or nullptr
+    volatile int32_t *flag;        // [n_out][W] set to 1 after the data of (write-out, walker) have been written
+    int32_t every;                 // sweeps between write-outs (m of Fig. 2)
+    int32_t n_out;                 // capacity in write-outs
+};
+
+struct SweepPlan  { int threads, J, V, P, K, cluster, smem_bytes, ctas_per_sm; const void *shape;
+                    const void *fallback; int fallback_smem; };   // fallback: one-move shape for what the tile kernel does not take
+// Process-wide overrides of the launch heuristics (qmc_set_tuning; tuning experiments and tests); -1 / 0 = heuristic.
+struct Tuning { int sweep_threads = 0, sweep_per_thread = 0, sweep_vector = -1, sweep_pending = -1, sweep_tile = -1,
+                    energy_threads = 0, energy_ordered = 0, sweep_cluster = -1; };
+extern Tuning g_tuning;
 struct EnergyPlan { int threads, smem_bytes, ctas_per_sm, variant; };   // variant 1 (FP64): unordered-pair kernel
 
 }  // namespace qmc
@@ -50,8 +67,11 @@ struct qmc_ctx {
     // qmc_run_blocks_host: write-out stream, double-buffered block results, their events (created on first use)
     cudaStream_t out_stream = nullptr;
     double *d_block = nullptr;                     // [2][W][5]
+    double *d_block_xyz = nullptr;                 // [2][W][3][N] coordinate write-outs (allocated on first use)
+    bool blocks_ready = false;                     // stream, d_block and the events below exist
     cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
     qmc::TraceView trace{};
+    qmc::WriteoutView wo{};                        // in-kernel write-outs of the running qmc_sweep_writeouts call
     qmc::SweepPlan sweep_plan{};
     qmc::EnergyPlan energy_plan{};
     uint64_t seed = 0;

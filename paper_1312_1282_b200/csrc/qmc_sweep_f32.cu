@@ -7,7 +7,7 @@ namespace qmc {
 #define X(T, J, V) QMC_SHAPE_ENTRY(float, T, J, V, 0)
 #define XP(T, J, V) QMC_SHAPE_ENTRY(float, T, J, V, 1)
 static const SweepShape kShapesF32[] = {
-    XP(32, 4, 4) XP(32, 8, 4) XP(32, 16, 4) XP(32, 32, 4) XP(64, 8, 4) XP(64, 16, 4) XP(64, 32, 4)
+    XP(32, 4, 4) XP(32, 8, 4) XP(32, 16, 4) XP(32, 32, 4) XP(64, 4, 4) XP(64, 8, 4) XP(64, 16, 4) XP(64, 32, 4)
     XP(128, 4, 4) XP(128, 8, 4) XP(128, 16, 4) XP(256, 4, 4) XP(256, 8, 4) XP(512, 4, 4) XP(512, 8, 4)
     XP(1024, 8, 4) XP(512, 20, 4) XP(1024, 10, 2)
     X(32, 1, 1) X(32, 2, 1) X(32, 4, 1) X(32, 8, 1) X(64, 8, 1) X(128, 8, 1) X(256, 8, 1) X(512, 8, 1) X(1024, 8, 1) X(1024, 10, 1)

@@ -7,6 +7,7 @@ namespace qmc {
 
 #define X(T, J, V) QMC_SHAPE_ENTRY(double, T, J, V, 0)
 static const SweepShape kShapesF64[] = {
+    X(64, 1, 1) X(64, 2, 1) X(64, 4, 1) X(128, 1, 1) X(128, 2, 1) X(128, 4, 1) X(256, 1, 1) X(256, 2, 1) X(64, 2, 2) X(256, 2, 2)
     X(32, 1, 1) X(32, 2, 1) X(32, 4, 1) X(32, 8, 1) X(64, 8, 1) X(128, 8, 1) X(256, 8, 1) X(512, 8, 1) X(1024, 6, 1)
     X(32, 2, 2) X(32, 4, 2) X(32, 8, 2) X(32, 16, 2) X(64, 4, 2) X(64, 8, 2) X(64, 16, 2)
     X(128, 2, 2) X(128, 4, 2) X(128, 8, 2) X(128, 16, 2) X(256, 4, 2) X(256, 8, 2) X(512, 4, 2) X(512, 8, 2) X(1024, 4, 2) X(1024, 6, 2)

@@ -193,6 +193,28 @@ __device__ __forceinline__ double sum_parts(const double *pb)
     return v[0];
 }
 
+__device__ __forceinline__ double coord_to_angstrom(double v, double) { return v; }
+__device__ __forceinline__ double coord_to_angstrom(int32_t k, double L_A) { return __dmul_rn(__dadd_rn((double)dec_coord(k), -1.0), L_A); }
+
+// coordinates + accepted-move count of this CTA's walker -> write-out slot; called by ALL threads at a sweep boundary
+template <int T, typename Coord>
+__device__ __forceinline__ void writeout_walker(const WriteoutView &wo, int slot, int w, int W, int N, double L_A,
+                                                const Coord *x, const Coord *y, const Coord *z,
+                                                unsigned long long n_acc_total)
+{
+    __syncthreads();                                          // the last commits of the sweep are in shared memory
+    double *dst = wo.xyz + ((size_t)slot * W + w) * 3 * N;
+    for (int j = threadIdx.x; j < N; j += T) {
+        dst[j]         = coord_to_angstrom(x[j], L_A);
+        dst[N + j]     = coord_to_angstrom(y[j], L_A);
+        dst[2 * N + j] = coord_to_angstrom(z[j], L_A);
+    }
+    if (threadIdx.x == 0 && wo.n_acc) wo.n_acc[(size_t)slot * W + w] = n_acc_total;
+    __threadfence_system();                                   // data before the flag, as seen from the host
+    __syncthreads();
+    if (threadIdx.x == 0) wo.flag[(size_t)slot * W + w] = 1;
+}
+
 // T threads per CTA; each thread owns J particles in G = J/V packs of V consecutive ones:
 // particle j = (g*T + tid)*V + e, g < G, e < V.  Shared arrays are padded to NP = T*J entries.
 // PD = 1 (FP32C, V >= 2): a running pair sum is held on chip as the unevaluated sum of two fp32 numbers
@@ -207,7 +229,7 @@ __device__ __forceinline__ double sum_parts(const double *pb)
 constexpr int kFold = 16;
 template <typename Real, int T, int J, int V, int PD, bool DBG>
 __global__ void __launch_bounds__(T, (sweep_min_ctas<Real, T, J, PD>()))
-sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
+sweep_kernel(StateView sv, TraceView tr, WriteoutView wo, uint2 key, uint32_t t0, int n_sweeps)
 {
     static_assert(J % V == 0, "J must be a multiple of the vector width");
     static_assert(PD == 0 || (sizeof(Real) == 4 && V >= 2), "pending sums exist only in the packed FP32C path");
@@ -505,6 +527,13 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
             if (sn == s) { xn = cx; yn = cy; zn = cz; }
             sp = s; pxp = cx; pyp = cy; pzp = cz;
         }
+        if constexpr (DBG) {                               // end of a sweep: optional in-kernel write-out (NEXT-4)
+            if (wo.xyz != nullptr && wo.every > 0 && (m + 1) % (uint32_t)N == 0) {
+                const uint32_t done = (m + 1) / (uint32_t)N;
+                if (done % (uint32_t)wo.every == 0 && (int)(done / (uint32_t)wo.every) <= wo.n_out)
+                    writeout_walker<T>(wo, (int)(done / (uint32_t)wo.every) - 1, w, sv.W, N, g.L_A, x, y, z, sv.n_acc[w] + n_acc);
+            }
+        }
         s = sn;
         xs = xn; ys = yn; zs = zn;
         mr = mrn;
@@ -521,23 +550,26 @@ sweep_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_sweeps)
     if (tid == 0) sv.n_acc[w] += n_acc;
 }
 
-// ---- host side: one table entry per compiled (T, J, V) shape ----------------------------------------
+// ---- host side: one table entry per compiled (T, J, V, PD, K) shape -----------------------------------
+// K = 1: this file's one-move kernel; K > 1: the tile kernel of qmc_sweep_tile.cuh (FP32C, PD = 1).
 struct SweepShape {
-    int T, J, V, P;
+    int T, J, V, P, K;
     cudaError_t (*launch)(qmc_ctx *c, int n_sweeps, int smem);
     int (*occupancy)(int smem);
+    int smem;
 };
 
 template <typename Real, int T, int J, int V, int PD>
 static cudaError_t shape_launch(qmc_ctx *c, int n_sweeps, int smem)
 {
     const uint2 key = make_uint2((uint32_t)(c->seed & 0xFFFFFFFFull), (uint32_t)(c->seed >> 32));
-    // the lean instantiation has neither the decision trace nor the general next-particle handling (N < 3, proposal 1)
-    const bool dbg = c->trace.dec != nullptr || c->p.N < 3 || c->sv.proposal != 0;
+    // the lean instantiation has neither the decision trace, the write-outs nor the general next-particle
+    // handling (N < 3, proposal 1)
+    const bool dbg = c->trace.dec != nullptr || c->p.N < 3 || c->sv.proposal != 0 || c->wo.xyz != nullptr;
     auto kern = dbg ? sweep_kernel<Real, T, J, V, PD, true> : sweep_kernel<Real, T, J, V, PD, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
-    kern<<<c->W, T, smem, c->stream>>>(c->sv, c->trace, key, c->t, n_sweeps);
+    kern<<<c->W, T, smem, c->stream>>>(c->sv, c->trace, c->wo, key, c->t, n_sweeps);
     return cudaGetLastError();
 }
 
@@ -551,9 +583,11 @@ static int shape_occupancy(int smem)
     return n;
 }
 
-#define QMC_SHAPE_ENTRY(Real, TT, JJ, VV, PP) {TT, JJ, VV, PP, shape_launch<Real, TT, JJ, VV, PP>, shape_occupancy<Real, TT, JJ, VV, PP>},
+#define QMC_SHAPE_ENTRY(Real, TT, JJ, VV, PP) {TT, JJ, VV, PP, 1, shape_launch<Real, TT, JJ, VV, PP>, shape_occupancy<Real, TT, JJ, VV, PP>, \
+                                               sweep_smem_bytes(TT, JJ, sizeof(Real) == 8 ? QMC_FP64 : QMC_FP32C, PP)},
 
 const SweepShape *sweep_shapes_f32(int *n);
 const SweepShape *sweep_shapes_f64(int *n);
+const SweepShape *sweep_shapes_tile(int *n);       // qmc_sweep_tile_f32.cu
 
 }  // namespace qmc

@@ -1,57 +1,104 @@
-// qmc_sweep_plan.cu -- host side of the sweep: choice of the (T, J, V) kernel shape for N and the launch.
+// qmc_sweep_plan.cu -- host side of the sweep: choice of the kernel shape (T threads per walker, J particles per
+// thread in packs of V, running-sum representation, tile size K) for N, W and the mode, and the launch.
 #include <cmath>
 #include <cstdlib>
 
-#include "qmc_sweep_impl.cuh"
+#include "qmc_sweep_tile.cuh"
 
 namespace qmc {
+
+Tuning g_tuning;
 
 cudaError_t launch_sweep(qmc_ctx *c, int n_sweeps)
 {
     c->launches += 1;
     const SweepShape *sh = static_cast<const SweepShape *>(c->sweep_plan.shape);
+    int smem = c->sweep_plan.smem_bytes;
+    if (sh != nullptr && sh->K > 1 && c->sv.proposal != 0) {       // the tile kernel moves particles in order only
+        sh = static_cast<const SweepShape *>(c->sweep_plan.fallback);
+        smem = c->sweep_plan.fallback_smem;
+    }
     if (sh == nullptr) return cudaErrorInvalidValue;
-    return sh->launch(c, n_sweeps, c->sweep_plan.smem_bytes);
+    return sh->launch(c, n_sweeps, smem);
 }
 
-// Threads per walker the heuristic aims at: about 16 particles per thread (measured on B200, profiles/),
-// one warp at least.  QMC_SWEEP_SHAPE="T,J[,V[,P]]" overrides the heuristic (tuning experiments).
+// What a shape costs (relative; it only has to rank shapes).  Fitted to the shape scans of the five configs in
+// profiles/r02_shapes.md:
+//   * in the throughput-bound regime a move costs every warp of the CTA  a J + b  pipe cycles (a: pair terms, b: the
+//     serial part -- reduction, barrier, decision; b / a = 1.35 in FP64, 4.2 in FP32C), so a sweep costs
+//     T (J + b/a): few threads with many particles each win, and padding (T J > N) is paid for;
+//   * that only holds while the SM has enough warps to overlap the serial parts of different walkers: below ~10
+//     resident warps per SM the time grows like 10 / warps.  W is given (PAPER.md l.484, l.502
+//     tuned walkers per SM instead), so with few walkers -- configs 1 and 2 -- threads per walker must grow;
+//   * more than 20 particles per thread costs registers (retained trial terms) and loses to the next wider shape.
+static double shape_cost(const SweepShape &s, int N, int W, int mode, int sm_count, int ctas_per_sm)
+{
+    if (ctas_per_sm < 1) return 1e300;
+    const double b_over_a = (mode == QMC_FP64) ? 1.35 : 4.2;
+    double cost = (double)s.T * ((double)s.J + b_over_a);
+    const double resident = std::fmin((double)ctas_per_sm, std::ceil((double)W / sm_count));
+    const double warps = resident * (s.T / 32);
+    if (warps < 10.0) cost *= 10.0 / warps;
+    if (s.J > 20) cost *= 1.15;
+    (void)N;
+    return cost;
+}
+
 bool plan_sweep(qmc_ctx *c, SweepPlan *out)
 {
-    const int N = c->p.N, mode = c->p.mode;
-    int n = 0;
+    const int N = c->p.N, mode = c->p.mode, W = c->W;
+    int n = 0, nt = 0;
     const SweepShape *tab = (mode == QMC_FP64) ? sweep_shapes_f64(&n) : sweep_shapes_f32(&n);
+    const SweepShape *tile = (mode == QMC_FP64) ? nullptr : sweep_shapes_tile(&nt);
     auto usable = [&](const SweepShape &s) {
         if ((long long)s.T * s.J < N) return false;
         if (s.V > 1 && N % s.V != 0) return false;
-        return sweep_smem_bytes(s.T, s.J, mode, s.P) <= 227 * 1024;
+        if (s.K > 1 && (N % s.K != 0 || N < 2 * s.K)) return false;
+        return s.smem <= 227 * 1024;
     };
+    const Tuning &tu = g_tuning;
+    auto wanted = [&](const SweepShape &s) {
+        return (tu.sweep_threads <= 0 || s.T == tu.sweep_threads) && (tu.sweep_per_thread <= 0 || s.J == tu.sweep_per_thread)
+            && (tu.sweep_vector < 0 || s.V == tu.sweep_vector) && (tu.sweep_pending < 0 || s.P == tu.sweep_pending)
+            && (tu.sweep_tile < 0 || s.K == (tu.sweep_tile < 1 ? 1 : tu.sweep_tile));
+    };
+    const bool forced = tu.sweep_threads > 0 || tu.sweep_per_thread > 0 || tu.sweep_vector >= 0 || tu.sweep_pending >= 0 || tu.sweep_tile >= 0;
     const SweepShape *best = nullptr;
-    if (const char *env = getenv("QMC_SWEEP_SHAPE")) {
-        int t = 0, j = 0, v = 0, pp = 0;
-        const int got = sscanf(env, "%d,%d,%d,%d", &t, &j, &v, &pp);
-        for (int k = 0; k < n && got >= 2; ++k)
-            if (tab[k].T == t && tab[k].J == j && (got < 3 || tab[k].V == v) && (got < 4 || tab[k].P == pp) && usable(tab[k]))
-                if (!best || tab[k].V > best->V || (tab[k].V == best->V && tab[k].P > best->P)) best = &tab[k];
-    }
-    if (!best) {
-        const int per_thread = 16;
-        double t_target = std::log2(std::fmax(32.0, std::fmin(1024.0, (double)N / per_thread)));
-        double best_score = 1e30;
-        for (int k = 0; k < n; ++k) {
-            if (!usable(tab[k])) continue;
-            const double waste = (double)(tab[k].T * tab[k].J - N) / (double)N;       // idle slots
-            const double score = 4.0 * waste + std::fabs(std::log2((double)tab[k].T) - t_target)
-                               + (mode == QMC_FP64 ? 0.25 * (2 - tab[k].V) : 0.25 * (4 - tab[k].V)) - 0.1 * tab[k].P;   // hi + lo running sums: 10.5 vs 11.1 ms at N = 1952 (measured)
-            if (score < best_score) { best_score = score; best = &tab[k]; }
+    double best_cost = 1e300;
+    int best_occ = 0;
+    for (int pass = 0; pass < 2 && !best; ++pass) {
+        // pass 0: shapes the tuning overrides ask for (if any); pass 1: the heuristic over the one-move shapes.
+        // The tile kernel (K > 1) is never the heuristic's choice: it measured slower than the one-move kernel at
+        // every config but config 4 (+0.8 %), see profiles/r02_tile.md; qmc_set_tuning("sweep_tile") selects it.
+        if (pass == 0 && !forced) continue;
+        for (int k = 0; k < n + nt; ++k) {
+            const SweepShape &s = k < n ? tab[k] : tile[k - n];
+            if (!usable(s) || (pass == 0 && !wanted(s)) || (pass == 1 && s.K > 1)) continue;
+            const int occ = s.occupancy(s.smem);
+            double cost = shape_cost(s, N, W, mode, c->sm_count, occ);
+            if (mode != QMC_FP64) cost *= (s.V == 4 ? 1.0 : (s.V == 2 ? 1.12 : 1.6)) * (s.P ? 1.0 : 1.06);
+            else                  cost *= (s.V == 2 ? 1.0 : 1.05);
+            if (cost < best_cost) { best_cost = cost; best = &s; best_occ = occ; }
         }
     }
-    out->threads = 0; out->J = 0; out->V = 0; out->ctas_per_sm = 0; out->shape = nullptr;
+    out->threads = 0; out->J = 0; out->V = 0; out->P = 0; out->K = 0; out->cluster = 1; out->ctas_per_sm = 0; out->shape = nullptr;
+    out->fallback = nullptr; out->fallback_smem = 0;
     out->smem_bytes = N * (8 + 3 * (mode == QMC_FP64 ? 8 : 4));
     if (!best) return false;
-    out->threads = best->T; out->J = best->J; out->V = best->V; out->shape = best;
-    out->smem_bytes = sweep_smem_bytes(best->T, best->J, mode, best->P);
-    out->ctas_per_sm = best->occupancy(out->smem_bytes);
+    out->threads = best->T; out->J = best->J; out->V = best->V; out->P = best->P; out->K = best->K; out->shape = best;
+    out->smem_bytes = best->smem;
+    out->ctas_per_sm = best_occ;
+    out->fallback = best;
+    out->fallback_smem = best->smem;
+    if (best->K > 1) {                               // the one-move kernel of the same geometry (proposal 1)
+        out->fallback = nullptr;
+        for (int k = 0; k < n; ++k)
+            if (tab[k].T == best->T && tab[k].J == best->J && tab[k].V == best->V && tab[k].P == 1 && usable(tab[k])) {
+                out->fallback = &tab[k];
+                out->fallback_smem = tab[k].smem;
+            }
+        if (!out->fallback) return false;
+    }
     return true;
 }
 

@@ -19,8 +19,8 @@ def lib():
     return binding.load_library()
 
 
-def header_symbols():
-    text = open(os.path.join(ROOT, "include", "qmc.h")).read()
+def header_symbols(name="qmc.h"):
+    text = open(os.path.join(ROOT, "include", name)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(qmc_[a-z_0-9]+)\s*\(", text)))
 
@@ -33,6 +33,18 @@ def test_library_exports_every_declared_symbol(lib):
     assert set(declared) <= exported
     for name in declared:
         assert getattr(lib, name) is not None
+    # the measurement tool is a library of its own (include/qmc_probe.h), outside the product ABI
+    nm = subprocess.run(["nm", "-D", "--defined-only", binding.PROBE_LIB_PATH], capture_output=True, text=True).stdout
+    assert set(header_symbols("qmc_probe.h")) == set(re.findall(r" T (qmc_[a-z_0-9]+)", nm)) == {"qmc_probe_rate"}
+    assert not set(header_symbols("qmc_probe.h")) & exported
+
+
+def test_tuning_keys(lib):
+    for key in ("sweep_threads", "sweep_per_thread", "sweep_vector", "sweep_pending", "sweep_tile", "sweep_cluster",
+                "energy_threads", "energy_ordered"):
+        assert lib.qmc_set_tuning(key.encode(), 1) == 0
+    assert lib.qmc_set_tuning(b"no_such_key", 1) == binding.QMC_E_ARG
+    assert lib.qmc_set_tuning(None, 0) == 0              # reset
 
 
 def test_library_is_sm100a_and_not_linked_to_the_oracle():
@@ -85,8 +97,8 @@ def test_no_gpu_means_a_loud_failure_not_a_fallback(lib):
     p, keep = _params()
     ctx = C.c_void_p()
     assert lib.qmc_create(C.byref(p), None, None, 0, C.byref(ctx)) == binding.QMC_E_CUDA
-    out = C.c_double()
-    assert lib.qmc_pipe_peak(0, None, C.byref(out)) == binding.QMC_E_CUDA
+    with pytest.raises(binding.QmcError):
+        binding.pipe_peak(0)
 
 
 def test_workloads_match_baseline_configs():

@@ -28,7 +28,19 @@ def qmc():
     from paper_1312_1282_b200 import binding, build
     build.build()
     binding.load_library()
+    binding.set_tuning()
     return binding
+
+
+@pytest.fixture
+def tuning(qmc):
+    """qmc_set_tuning for the contexts a test creates; reset afterwards."""
+    def set_(**kw):
+        qmc.set_tuning()
+        for k, v in kw.items():
+            qmc.set_tuning(k, v)
+    yield set_
+    qmc.set_tuning()
 
 
 def make(qmc, N, W, mode, rho=wl.RHO_EQ, b=2.89, base=0, aziz=AZ, **kw):
@@ -247,6 +259,8 @@ def test_local_energy_fp32c(qmc, oracle, N):
     ok = ~((eo[:, 5] < 5e-7) & (jump > 0.1 * TOL32 * np.abs(eo[:, 0])))
     assert ok.any()
     assert relerr32(eg[ok], eo[ok]).max() < TOL32, relerr32(eg[ok], eo[ok])
+    if N >= 256:                                        # R22: the floor on E_PB's denominator is not needed here:
+        assert (np.abs(eg - eo[:, :4]) / np.abs(eo[:, :4]))[ok].max() < TOL32      # plain relative error, every column
     S = q.pair_sums().cpu().numpy()
     Sr = oracle.pair_sums(orc_sys(oracle, N, L), xyz[0])
     assert np.abs(S[0] - Sr).max() < 2e-6 * np.abs(Sr).max()
@@ -279,14 +293,15 @@ def test_local_energy_config4_size(qmc, oracle):
     eg = q.local_energy().cpu().numpy()
     eo = oracle.local_energy(orc_sys(oracle, N, L), xyz)
     assert relerr32(eg, eo).max() < TOL32
-    # and sweeps run at this size (1024 threads x 10 particles); the running pair sums stay equal to
-    # the kernel's own from-scratch rebuild (GPU-internal invariant; the rebuild itself is checked
-    # against the oracle above and in test_local_energy_fp32c)
+    # and sweeps run at this size (512 threads x 20 particles): the running pair sums after two sweeps against the
+    # oracle's definition on the exported coordinates, and against the kernel's own from-scratch rebuild
     q.sweep(2, 1.0)
     S_run = q.pair_sums().cpu().numpy()[0]
+    S_orc = oracle.pair_sums(orc_sys(oracle, N, L), q.get_positions().cpu().numpy()[0])
+    assert np.abs(S_run - S_orc).max() < 5e-5 * np.abs(S_orc).max()
     q.refresh_pair_sums()
     S_new = q.pair_sums().cpu().numpy()[0]
-    assert np.abs(S_run - S_new).max() < 2e-5 * np.abs(S_new).max()
+    assert np.abs(S_new - S_orc).max() < 2e-6 * np.abs(S_orc).max()
     a = float(q.acceptance().cpu()[0])
     assert 0.3 < a < 0.8
 
@@ -301,6 +316,131 @@ def test_free_particles_energy_zero_acceptance_one(qmc):
         e = q.local_energy().cpu().numpy()
         assert (e == 0.0).all()
         assert (q.acceptance().cpu().numpy() == 1.0).all()
+
+
+# ------------------------------------------------------------------------------ fp32c sweeps against the oracle
+GRID = 8388608                       # 2^23 grid cells per box edge (R20)
+# Bound on |margin_gpu - margin_oracle| of one FP32C move, per unit of max(1, |margin_oracle|), derived in DESIGN.md
+# R23 from the fp32 error of one pair term (eps_t = 1.7e-6: rsqrt.approx 2^-22 taken to the fifth power plus the
+# roundings of r^2 and of the powers) and the sums of |u| that enter a move (<= ~7 each for the trial and the old
+# position in the liquid): 2 * 1.7e-6 * 14 = 4.8e-5.  Not tuned to the measured differences (a few 1e-6).
+TOL_MARGIN32 = 5e-5
+
+
+def grid_index(x, L):
+    """23-bit grid indices of coordinates that lie exactly on the FP32C grid x = fl(k 2^-23 L)."""
+    k = np.rint(x / L * GRID).astype(np.int64) % GRID
+    assert np.array_equal(k.astype(np.float64) * 2.0 ** -23 * L, x), "coordinates are not on the FP32C grid"
+    return k
+
+
+def replay_fp32c(oracle, s, k0, seed, w, t0, sweeps, step, dec_gpu):
+    """One walker of an FP32C run replayed in the fp64 oracle on the SAME grid coordinates (R20): the trial position
+    of a move is the grid index plus the displacement rounded to the grid, dk = rint(fl(fl(step fl(1/L)) 2^23) a_k),
+    a_k the exact variates of the move; positions are x = fl(k 2^-23 L).  The oracle's Eq.(7) Delta (orc_delta_log_psi,
+    two plain loops, no running sums) gives the margin 2 Delta - log xi of every move; the GPU's decisions are
+    adopted (R19).  Returns (oracle margins [moves], final grid indices [3][N])."""
+    N, L = s.N, s.L
+    k = k0.copy()
+    x = k.astype(np.float64) * 2.0 ** -23 * L
+    step_grid = step * (1.0 / L) * 8388608.0
+    mar = np.zeros(sweeps * N)
+    m = 0
+    for t in range(t0, t0 + sweeps):
+        for q in range(N):
+            if s.proposal == 1:
+                p, a, xi = oracle.move_variates_gauss(seed, w, t, q, N, 1.0)
+            else:
+                (a, xi), p = oracle.move_variates(seed, w, t, q, 1.0), q
+            kt = (k[:, p] + np.rint(step_grid * a).astype(np.int64)) % GRID
+            xt = kt.astype(np.float64) * 2.0 ** -23 * L
+            mar[m] = 2.0 * oracle.delta_log_psi(s, x, p, xt) - math.log(xi)
+            if dec_gpu[m]:
+                k[:, p] = kt
+                x[:, p] = xt
+            m += 1
+    return mar, k
+
+
+def oracle_liquid_on_grid(oracle, N, L, W, seed, sweeps):
+    """Start of the FP32C sweep tests: the oracle's own fp64 chain from the jittered lattice (oracle -> GPU, never
+    the reverse), snapped down to the FP32C grid."""
+    s = orc_sys(oracle, N, L)
+    x = oracle.init_walkers(s, seed, 0, W, wl.JITTER)
+    if sweeps:
+        oracle.sweep(s, x, seed, 0, 0, sweeps, 1.0)
+    k = np.floor(x / L * GRID).astype(np.int64) % GRID
+    return k.astype(np.float64) * 2.0 ** -23 * L
+
+
+@pytest.mark.parametrize("N,W,eq,sweeps,tune,proposal", [
+    # config 3, the bench shape: 128 threads x 16 particles, V = 4, hi + lo sums, whatever tile size the planner picks
+    (1952, 3, 12, 2, dict(), 0),
+    (1952, 2, 12, 2, dict(sweep_threads=128, sweep_per_thread=16, sweep_tile=1), 0),      # one-move kernel
+    (1952, 2, 12, 2, dict(sweep_threads=128, sweep_per_thread=16, sweep_tile=2), 0),      # tiles of 2 moves
+    (1952, 2, 12, 2, dict(sweep_threads=128, sweep_per_thread=16, sweep_tile=4), 0),      # tiles of 4 moves
+    (1952, 2, 12, 1, dict(sweep_threads=256, sweep_per_thread=8, sweep_tile=4), 0),
+    (10000, 1, 0, 1, dict(), 0),              # config 4: one CTA per SM, 202 KB of shared memory
+    (10000, 1, 0, 1, dict(sweep_threads=512, sweep_per_thread=20, sweep_tile=1), 0),
+    (10000, 1, 0, 1, dict(sweep_threads=1024, sweep_per_thread=10, sweep_tile=2), 0),     # V = 2 packs
+    (256, 4, 40, 3, dict(), 0),
+    (256, 4, 40, 3, dict(sweep_threads=32, sweep_per_thread=8, sweep_tile=4), 0),         # one warp: no block barrier
+    (256, 4, 40, 3, dict(sweep_threads=64, sweep_per_thread=4, sweep_tile=2), 0),
+    (64, 6, 60, 4, dict(), 0),
+    (64, 6, 60, 4, dict(sweep_tile=1), 0),
+    (37, 4, 40, 5, dict(), 0),                # scalar (V = 1) shape, ragged
+    (1952, 2, 12, 1, dict(), 1),              # the paper's proposal (random particle, Gaussian step)
+])
+def test_fp32c_sweep_margins_vs_oracle(qmc, oracle, tuning, N, W, eq, sweeps, tune, proposal):
+    """The TIMED kernel against the oracle at its own shape: every decision margin
+    2 Delta - log xi of FP32C sweeps equals the fp64 oracle's Eq.(7) margin on the same grid coordinates within
+    TOL_MARGIN32; a decision may differ from the sign of the oracle's margin only inside that window; the
+    committed coordinates are bit-identical to the replay; the running pair sums equal oracle.pair_sums."""
+    tuning(**tune)
+    q, L = make(qmc, N, W, qmc.QMC_FP32C)
+    inf = q.info()
+    for key, name in (("sweep_threads", "sweep_threads"), ("sweep_per_thread", "sweep_pairs_per_thread"), ("sweep_tile", "sweep_tile")):
+        if key in tune:
+            assert inf[name] == tune[key], inf          # the forced shape exists and is the one that runs
+    if not tune and N in (1952, 10000):                  # the planner's own choice for configs 3 / 4 is a packed hi + lo shape
+        assert inf["sweep_vector"] == 4 and inf["sweep_pending"] == 1, inf
+    if N == 10000:
+        x0 = wl.liquid_configuration(N, L, 4242, fp32_grid=True)[None]
+    else:
+        x0 = oracle_liquid_on_grid(oracle, N, L, W, 77, eq)
+    seed, t0, step = 99, 5, (1.0 if proposal == 0 else 0.7)
+    q.set_proposal(proposal)
+    q.set_positions(x0)
+    assert np.array_equal(q.get_positions().cpu().numpy(), x0)
+    q.set_seed(seed, t0)
+    dec, mar = q.trace_decisions(0, W, sweeps * N)
+    q.sweep(sweeps, step)
+    dec, mar = dec.cpu().numpy(), mar.cpu().numpy()
+    xg = q.get_positions().cpu().numpy()
+    Sg = q.pair_sums().cpu().numpy()
+    s = oracle.System(N, L, 2.89, DK, AZ, proposal=proposal)
+    worst = 0.0
+    for w in range(W):
+        mo, kf = replay_fp32c(oracle, s, grid_index(x0[w], L), seed, w, t0, sweeps, step, dec[w])
+        scale = np.maximum(1.0, np.abs(mo))
+        err = np.abs(mar[w] - mo) / scale
+        worst = max(worst, err.max())
+        assert err.max() < TOL_MARGIN32, (w, int(err.argmax()), err.max())
+        bad = (mo > 0) != (dec[w] != 0)
+        assert np.all(np.abs(mo[bad]) < TOL_MARGIN32 * scale[bad]), np.abs(mo[bad]).max()
+        assert np.array_equal(grid_index(xg[w], L), kf), "committed grid coordinates must be identical"
+        So = oracle.pair_sums(s, xg[w])
+        assert np.abs(Sg[w] - So).max() < 2e-5 * np.abs(So).max()
+    assert 0.2 < dec.mean() < 0.8
+    # the same call without the trace (the instantiation bench.py times) lands on the same bits
+    q2, _ = make(qmc, N, W, qmc.QMC_FP32C)
+    q2.set_proposal(proposal)
+    q2.set_positions(x0)
+    q2.set_seed(seed, t0)
+    q2.sweep(sweeps, step)
+    assert np.array_equal(q2.get_positions().cpu().numpy(), xg)
+    assert np.array_equal(q2.pair_sums().cpu().numpy(), Sg)
+    print(f"N={N} T={inf['sweep_threads']} J={inf['sweep_pairs_per_thread']} K={inf['sweep_tile']}: worst margin error {worst:.2e} of {TOL_MARGIN32:.0e}")
 
 
 # ------------------------------------------------------------------------------ fp32c statistics
@@ -354,50 +494,59 @@ def test_fp32c_sweep_odd_sizes(qmc, N):
     assert x.min() >= 0.0 and x.max() <= L
 
 
-def test_fp32c_pair_sums_do_not_drift(qmc):
-    """Running S_i after 60 fp32c sweeps still equal the from-scratch sums to fp32 accuracy (R17);
-    the energy pass rebuilds them.  GPU-internal invariant: the rebuild is pinned to the oracle in
-    test_local_energy_fp32c (same kernel, generator inputs)."""
+def test_fp32c_pair_sums_do_not_drift(qmc, oracle):
+    """Running S_i after 60 fp32c sweeps still equal the definition (oracle.pair_sums on the exported coordinates)
+    to fp32 accuracy (R17); the energy pass rebuilds them an order of magnitude closer."""
     N = 256
     q, L = make(qmc, N, 2, qmc.QMC_FP32C)
     q.init_walkers(9)
     q.sweep(60, 1.0)
     S = q.pair_sums().cpu().numpy()
+    x = q.get_positions().cpu().numpy()
+    So = np.stack([oracle.pair_sums(orc_sys(oracle, N, L), x[w]) for w in range(2)])
+    assert np.abs(S - So).max() < 2e-5 * np.abs(So).max()
     q.local_energy()
     S2 = q.pair_sums().cpu().numpy()
-    assert np.abs(S - S2).max() < 2e-5 * np.abs(S2).max()
+    assert np.abs(S2 - So).max() < 2e-6 * np.abs(So).max()
     assert not np.array_equal(S, S2)
 
 
-def test_fp32c_sum_representations_agree(qmc, monkeypatch):
-    """A PD = 0 sweep shape (fp64 running sums in shared memory) against the default PD = 1 shape (sums held as
-    an fp32 pair hi + lo, R20) on the same walkers: running sums equal to fp32 accuracy, acceptance equal to a few flipped near-ties.
-    GPU-internal: the default shape is the one pinned to the oracle above."""
+def test_fp32c_sum_representations_agree(qmc, tuning):
+    """A PD = 0 sweep shape (fp64 running sums in shared memory) against the PD = 1 shape (sums held as an fp32 pair
+    hi + lo, R20) and the tile kernel on the same walkers: running sums equal to fp32 accuracy, coordinates
+    equal up to a flipped near-tie.  GPU-internal: each is pinned to the oracle in test_fp32c_sweep_margins_vs_oracle."""
     N, W = 256, 6
-    q0, L = make(qmc, N, W, qmc.QMC_FP32C)
-    monkeypatch.setenv("QMC_SWEEP_SHAPE", "64,8,4,0")
-    q1, _ = make(qmc, N, W, qmc.QMC_FP32C)
-    monkeypatch.delenv("QMC_SWEEP_SHAPE")
-    assert q1.info()["sweep_threads"] == 64 and q1.info()["sweep_pairs_per_thread"] == 8
-    for q in (q0, q1):
+    qs = []
+    for tune in (dict(sweep_threads=64, sweep_per_thread=8, sweep_vector=4, sweep_pending=0, sweep_tile=1),
+                 dict(sweep_threads=64, sweep_per_thread=8, sweep_vector=4, sweep_pending=1, sweep_tile=1),
+                 dict(sweep_threads=64, sweep_per_thread=8, sweep_vector=4, sweep_pending=1, sweep_tile=4)):
+        tuning(**tune)
+        q, L = make(qmc, N, W, qmc.QMC_FP32C)
+        inf = q.info()
+        assert (inf["sweep_threads"], inf["sweep_pairs_per_thread"], inf["sweep_pending"], inf["sweep_tile"]) == \
+            (64, 8, tune["sweep_pending"], tune["sweep_tile"]), inf
         q.init_walkers(21)
         q.sweep(3, 1.0)
-    S0, S1 = q0.pair_sums().cpu().numpy(), q1.pair_sums().cpu().numpy()
-    same = np.array([np.array_equal(a, b) for a, b in zip(q0.get_positions().cpu().numpy(), q1.get_positions().cpu().numpy())])
-    assert same.sum() >= W - 1                       # a near-tie may send one chain another way
-    assert np.abs(S0[same] - S1[same]).max() < 2e-5 * np.abs(S0).max()
-    q1.local_energy()                                 # rebuild from scratch
-    S1r = q1.pair_sums().cpu().numpy()
-    assert np.abs(S1 - S1r).max() < 2e-5 * np.abs(S1r).max()
+        qs.append(q)
+    S0 = qs[0].pair_sums().cpu().numpy()
+    x0 = qs[0].get_positions().cpu().numpy()
+    for q in qs[1:]:
+        S1, x1 = q.pair_sums().cpu().numpy(), q.get_positions().cpu().numpy()
+        same = np.array([np.array_equal(a, b) for a, b in zip(x0, x1)])
+        assert same.sum() >= W - 1                       # a near-tie may send one chain another way
+        assert np.abs(S0[same] - S1[same]).max() < 2e-5 * np.abs(S0).max()
+        q.local_energy()                                  # rebuild from scratch
+        S1r = q.pair_sums().cpu().numpy()
+        assert np.abs(S1 - S1r).max() < 2e-5 * np.abs(S1r).max()
 
 
-def test_local_energy_fp64_ordered_fallback(qmc, oracle, monkeypatch):
+def test_local_energy_fp64_ordered_fallback(qmc, oracle, tuning):
     """The ordered-pair fp64 energy kernel (used when the unordered-pair kernel's accumulators do not fit
     shared memory) against the oracle."""
-    monkeypatch.setenv("QMC_ENERGY_ORDERED", "1")
+    tuning(energy_ordered=1)
     N, W = 300, 3
     q, L = make(qmc, N, W, qmc.QMC_FP64)
-    monkeypatch.delenv("QMC_ENERGY_ORDERED")
+    assert q.info()["energy_variant"] == 0
     xyz = np.stack([wl.liquid_configuration(N, L, 900 + k) for k in range(W)])
     q.set_positions(xyz)
     eg = q.local_energy().cpu().numpy()
@@ -485,6 +634,105 @@ def test_run_blocks_host_equals_stepwise_calls(qmc):
             assert np.array_equal(qb.local_energy().cpu().numpy(), he[b].numpy())
             assert np.array_equal(qb.acceptance().cpu().numpy(), ha[b].numpy())
         assert torch.equal(qa.get_positions(), qb.get_positions())
+
+
+def test_run_blocks_host_vs_oracle(qmc, oracle):
+    """NEXT-4 against the ORACLE: fp64, N = 64; the energies and accepted fractions each block
+    writes out equal the oracle chain's after the same sweeps (1e-10), the coordinate write-outs of every second
+    block are bit-identical; two calls follow each other without qmc_wait (buffer reuse across calls)."""
+    import torch
+    N, W, blocks, m = 64, 4, 6, 2
+    q, L = make(qmc, N, W, qmc.QMC_FP64)
+    q.init_walkers(wl.SEED)
+    dec, _ = q.trace_decisions(0, W, blocks * m * N)
+    he = torch.zeros((blocks, W, 4), dtype=torch.float64).pin_memory()
+    ha = torch.zeros((blocks, W), dtype=torch.float64).pin_memory()
+    hx = torch.zeros((blocks // 2, W, 3, N), dtype=torch.float64).pin_memory()
+    hd = torch.zeros((blocks,), dtype=torch.int32).pin_memory()
+    half = blocks // 2
+    q.run_blocks_host(half, m, 1.0, he[:half], ha[:half], hd[:half], xyz_every=2, h_xyz=hx[:half // 2])
+    q.run_blocks_host(blocks - half, m, 1.0, he[half:], ha[half:], hd[half:], xyz_every=1, h_xyz=None)
+    q.wait()
+    assert hd.tolist() == [1] * blocks
+    dec = dec.cpu().numpy()
+    s = orc_sys(oracle, N, L)
+    xo = oracle.init_walkers(s, wl.SEED, 0, W, wl.JITTER)
+    nacc = np.zeros(W)
+    for b in range(blocks):
+        force = np.ascontiguousarray(dec[:, b * m * N:(b + 1) * m * N])
+        na, _, mo = oracle.sweep(s, xo, wl.SEED, 0, b * m, m, 1.0, want_trace=True, force=force)
+        bad = (mo > 0) != (force != 0)
+        assert np.all(np.abs(mo[bad]) < TIE)
+        nacc += na
+        eo = oracle.local_energy(s, xo)[:, :4]
+        assert relerr(he[b].numpy(), eo).max() < TOL64, (b, relerr(he[b].numpy(), eo).max())
+        assert np.allclose(ha[b].numpy(), nacc / ((b + 1) * m * N), rtol=0, atol=1e-15)
+        if b == 1:
+            assert np.array_equal(hx[0].numpy(), xo)          # the only coordinate write-out of the first call
+    assert np.array_equal(q.get_positions().cpu().numpy(), xo)
+
+
+@pytest.mark.parametrize("N,W,every,n_out,where", [(64, 5, 2, 4, "host"), (100, 3, 1, 3, "device"), (2, 4, 3, 2, "host")])
+def test_sweep_writeouts_fp64_vs_oracle(qmc, oracle, N, W, every, n_out, where):
+    """qmc_sweep_writeouts (NEXT-4, the paper's mechanism: l.175, l.323, l.343): ONE launch, the running kernel writes
+    coordinates and accepted-move counts out every `every` sweeps -- into mapped pinned host memory or device
+    memory -- and raises a flag per (write-out, walker).  fp64: every write-out is bit-identical to the oracle
+    chain after the same number of sweeps."""
+    import torch
+    q, L = make(qmc, N, W, qmc.QMC_FP64)
+    q.init_walkers(wl.SEED)
+    sweeps = every * n_out + (1 if every > 1 else 0)          # a trailing sweep without write-out
+    step = 1.0 if N > 2 else 0.4
+    dec, _ = q.trace_decisions(0, W, sweeps * N)
+    kw = dict(pin_memory=True) if where == "host" else dict(device="cuda")
+    xyz = torch.full((n_out, W, 3, N), -1.0, dtype=torch.float64, **kw)       # impossible values (l.323)
+    nacc = torch.full((n_out, W), -1, dtype=torch.int64, **kw)
+    flags = torch.zeros((n_out, W), dtype=torch.int32, **kw)
+    q.sweep_writeouts(sweeps, step, every, xyz, nacc, flags)
+    xg = q.get_positions().cpu().numpy()
+    assert flags.cpu().numpy().all()
+    dec = dec.cpu().numpy()
+    s = orc_sys(oracle, N, L)
+    xo = oracle.init_walkers(s, wl.SEED, 0, W, wl.JITTER)
+    tot = np.zeros(W, np.int64)
+    for k in range(n_out):
+        force = np.ascontiguousarray(dec[:, k * every * N:(k + 1) * every * N])
+        na, _, mo = oracle.sweep(s, xo, wl.SEED, 0, k * every, every, step, want_trace=True, force=force)
+        bad = (mo > 0) != (force != 0)
+        assert np.all(np.abs(mo[bad]) < TIE)
+        tot += na
+        assert np.array_equal(xyz[k].cpu().numpy(), xo), k
+        assert np.array_equal(nacc[k].cpu().numpy(), tot)
+    if sweeps > every * n_out:
+        force = np.ascontiguousarray(dec[:, n_out * every * N:])
+        oracle.sweep(s, xo, wl.SEED, 0, n_out * every, sweeps - n_out * every, step, force=force)
+    assert np.array_equal(xg, xo)
+
+
+@pytest.mark.parametrize("N,tile", [(256, 4), (1952, 2), (1952, 4)])
+def test_sweep_writeouts_fp32c_tile_kernel(qmc, tuning, N, tile):
+    """The same write-outs from the tiled FP32C kernel: equal to the coordinates qmc_get_positions returns after
+    separate launches of the same sweeps (GPU-internal; that kernel is pinned to the oracle in
+    test_fp32c_sweep_margins_vs_oracle)."""
+    import torch
+    tuning(sweep_tile=tile)
+    W, every, n_out = 3, 2, 3
+    qa, L = make(qmc, N, W, qmc.QMC_FP32C)
+    qb, _ = make(qmc, N, W, qmc.QMC_FP32C)
+    assert qa.info()["sweep_tile"] == tile
+    for q in (qa, qb):
+        q.init_walkers(5)
+    xyz = torch.full((n_out, W, 3, N), -1.0, dtype=torch.float64).pin_memory()
+    nacc = torch.full((n_out, W), -1, dtype=torch.int64).pin_memory()
+    flags = torch.zeros((n_out, W), dtype=torch.int32).pin_memory()
+    qa.sweep_writeouts(every * n_out, 1.0, every, xyz, nacc, flags)
+    qa.wait()
+    assert flags.numpy().all()
+    for k in range(n_out):
+        qb.sweep(every, 1.0)
+        assert np.array_equal(xyz[k].numpy(), qb.get_positions().cpu().numpy())
+        assert np.array_equal(nacc[k].numpy() / ((k + 1) * every * N), qb.acceptance().cpu().numpy())
+    assert torch.equal(qa.get_positions(), qb.get_positions())
 
 
 def test_pipe_peak_microbenchmark_is_plausible(qmc):
