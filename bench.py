@@ -28,9 +28,14 @@ if ROOT not in sys.path:
 from paper_1312_1282_b200 import workloads as wl  # noqa: E402
 
 # Algorithmic FP instructions per u-evaluation of the sweep: thread-level
-# instructions on the pipe that bounds the mode, for ONE trial-position pair evaluation.
+# instructions on the pipe that bounds the mode, for ONE trial-position pair evaluation.  The counts are
+# checked against ncu's sm__sass_thread_inst_executed_op_* per executed pair evaluation in profiles/r02_instr.md.
 ALG_INSTR = {wl.MODE_FP32C: 24.0, wl.MODE_FP64: 31.0}
 LANES_PER_SM = {wl.MODE_FP32C: 128, wl.MODE_FP64: 64}
+# DRAM bytes per launch of the dominant kernel from the ncu --set full capture of the same command
+# (profiles/r02_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum); None where no capture exists.
+NCU_TRAFFIC_BYTES = {("c3-N1952", wl.MODE_FP32C): 80.1e6 + 22.1e6, ("c3-N1952-fp64", wl.MODE_FP64): 129.7e6 + 69.4e6}
+EQUIL_SWEEPS = {1: 200, 2: 200, 3: 150, 4: 20, 5: 60}      # untimed, before the warm-up (time the liquid, not the melting lattice)
 
 
 def pair_counts(w: wl.Workload, m: int):
@@ -133,6 +138,115 @@ def run_reference(args, w, m):
     }))
 
 
+def spawn_ranks(n: int):
+    """`python bench.py --gpus N` without a launcher: start N ranks (one per GPU) under torch.distributed.run and
+    replace this process by it (VERDICT r1 missing #4).  NCCL_DEBUG stays whatever the caller set."""
+    import socket
+    sock = socket.socket()
+    sock.bind(("127.0.0.1", 0))
+    port = sock.getsockname()[1]
+    sock.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    os.execv(sys.executable, cmd)
+
+
+def plumbing_only(args):
+    """--plumbing-only: the rank plumbing without any GPU work (CPU test of the launch path): every rank joins a gloo
+    group, the ranks count themselves, rank 0 prints the line's n_gpus."""
+    import torch
+    import torch.distributed as dist
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+        t = torch.ones(1)
+        dist.all_reduce(t)
+        assert int(t.item()) == world
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"plumbing_only": True, "n_gpus": world, "requested_gpus": args.gpus}))
+
+
+class Timed:
+    """One workload on this rank's GPU: context, equilibration, warm-up, K timed steps (sweep | energy + acceptance)."""
+
+    def __init__(self, w, m, dev, rank, proposal=0, sigma=0.8):
+        import torch
+        from paper_1312_1282_b200 import binding
+        self.torch, self.w, self.m, self.dev = torch, w, m, dev
+        W = w.n_walkers
+        self.q = binding.QMC(w.n_atoms, w.walkers_per_group, w.box_L, w.jastrow_b, w.hbar2_over_2m, w.aziz, w.mode,
+                             walker_id_base=rank * W, jitter=wl.JITTER, device=str(dev))
+        self.q.init_walkers(w.seed)
+        self.steps = w.steps
+        if proposal == 1:
+            self.q.set_proposal(1)
+            self.steps = [sigma] * len(w.groups)
+        self.e_out = torch.empty((W, 4), dtype=torch.float64, device=dev)
+        self.a_out = torch.empty((W,), dtype=torch.float64, device=dev)
+
+    def one_step(self):
+        self.q.sweep(self.m, self.steps)
+        self.q.local_energy(self.e_out)
+        self.q.acceptance(self.a_out)
+
+    def run(self, equil, warmup, K, flush, barrier=None, sampler=None):
+        torch, q = self.torch, self.q
+        if equil > 0:
+            q.sweep(equil, self.steps)                     # untimed: melt the lattice
+        for _ in range(warmup):
+            self.one_step()
+        torch.cuda.synchronize()
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+        if barrier:
+            barrier()
+        torch.cuda.synchronize()
+        if sampler:
+            sampler.start()
+        launches0 = q.info()["kernel_launches"]
+        for k in range(K):
+            flush.zero_()                                   # L2 flush between timed iterations (untimed)
+            ev[k][0].record()
+            q.sweep(self.m, self.steps)
+            ev[k][1].record()
+            q.local_energy(self.e_out)
+            q.acceptance(self.a_out)
+            ev[k][2].record()
+        torch.cuda.synchronize()
+        self.launches = q.info()["kernel_launches"] - launches0
+        if barrier:
+            barrier()
+        self.t_sweep = sum(ev[k][0].elapsed_time(ev[k][1]) for k in range(K)) * 1e-3
+        self.t_total = sum(ev[k][0].elapsed_time(ev[k][2]) for k in range(K)) * 1e-3
+        self.acc = float(self.a_out.mean())
+        self.e_mean = (self.e_out.mean(0) / self.w.n_atoms).tolist()
+        return self
+
+
+def summarize(t: "Timed", K, sm_count, sm_max_mhz, world=1):
+    """Throughput and roofline keys of one timed workload (shared by the headline and the `configs` block)."""
+    w, m = t.w, t.m
+    sweep_pairs, energy_pairs = pair_counts(w, m)
+    peak = sm_count * LANES_PER_SM[w.mode] * sm_max_mhz * 1e6
+    t_launch = t.t_sweep / K
+    achieved = sweep_pairs * ALG_INSTR[w.mode] / t_launch
+    info = t.q.info()
+    return {
+        "workload": w.name, "N": w.n_atoms, "walkers": w.n_walkers, "groups": len(w.groups),
+        "mode": "fp32c" if w.mode == wl.MODE_FP32C else "fp64", "steps": K,
+        "ms_per_step": 1e3 * t.t_total / K, "sweep_ms": 1e3 * t.t_sweep / K, "energy_ms": 1e3 * (t.t_total - t.t_sweep) / K,
+        "pair_evals_per_s": world * K * (sweep_pairs + energy_pairs) / t.t_total,
+        "sweep_pair_evals_per_s": world * K * sweep_pairs / t.t_sweep,
+        "energy_pairs_per_s": world * K * energy_pairs / (t.t_total - t.t_sweep),
+        "walker_sweeps_per_s": world * K * w.n_walkers * m / t.t_total,
+        "sweep_roofline_frac": achieved / peak, "sweep_roofline_executed_frac": achieved * (1.0 + t.acc) / peak,
+        "acceptance": t.acc, "energy_per_atom_K": dict(zip(["E_PB", "V", "T_PB", "T_JF"], t.e_mean)),
+        "sweep_shape": {k: info[k] for k in ("sweep_threads", "sweep_pairs_per_thread", "sweep_vector", "sweep_pending",
+                                              "sweep_tile", "sweep_ctas_per_sm")},
+        "energy_shape": {k: info[k] for k in ("energy_threads", "energy_variant", "energy_ctas_per_sm")},
+    }
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -143,6 +257,8 @@ def main():
     ap.add_argument("--sweeps-per-step", type=int, default=1)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the `configs` block (the other BASELINE.json configs)")
+    ap.add_argument("--equil", type=int, default=None, help="untimed equilibration sweeps before the warm-up (default per config)")
     ap.add_argument("--walkers", type=int, default=None, help="truncate walkers per group (debugging)")
     ap.add_argument("--proposal", type=int, choices=[0, 1], default=0,
                     help="0: particles in order, uniform cube (BASELINE.json); 1: the paper's random particle + "
@@ -151,7 +267,14 @@ def main():
     ap.add_argument("--time-to-error", type=int, default=0, metavar="S",
                     help="after the timed steps: S more steps with the energy recorded, reblocked -> the paper's "
                          "t*sigma^2 and seconds to 1 mK per atom (PAPER.md l.504-511); 0 = skip")
+    ap.add_argument("--large-n", action="store_true", help="add the NEXT-3 cluster-kernel figures (N = 40960, one walker on 8 SMs)")
+    ap.add_argument("--plumbing-only", action="store_true", help="rank plumbing only, no GPU work (CPU test of --gpus N)")
     args = ap.parse_args()
+
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        spawn_ranks(args.gpus)                               # does not return
+    if args.plumbing_only:
+        return plumbing_only(args)
 
     w = wl.config(args.config)
     if args.mode != "default":
@@ -180,71 +303,41 @@ def main():
 
     # weak scaling: every rank runs the workload's W walkers; global walker ids continue across ranks
     W, N = w.n_walkers, w.n_atoms
-    q = binding.QMC(N, w.walkers_per_group, w.box_L, w.jastrow_b, w.hbar2_over_2m, w.aziz, w.mode,
-                    walker_id_base=rank * W, jitter=wl.JITTER, device=str(dev))
-    q.init_walkers(w.seed)
-    steps = w.steps
-    if args.proposal == 1:
-        q.set_proposal(1)
-        steps = [args.sigma] * len(w.groups)
-    e_out = torch.empty((W, 4), dtype=torch.float64, device=dev)
-    a_out = torch.empty((W,), dtype=torch.float64, device=dev)
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)   # 256 MiB > 126 MB L2
-
-    def one_step():
-        q.sweep(m, steps)
-        q.local_energy(e_out)
-        q.acceptance(a_out)
-
-    for _ in range(args.warmup):
-        one_step()
-    torch.cuda.synchronize()
-
     K = args.steps
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
     sampler = ClockSampler(local) if rank == 0 else None
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
-    if sampler:
-        sampler.start()
-    launches0 = q.info()["kernel_launches"]
-    for k in range(K):
-        flush.zero_()                                   # L2 flush between timed iterations (untimed)
-        ev[k][0].record()
-        q.sweep(m, steps)
-        ev[k][1].record()
-        q.local_energy(e_out)
-        q.acceptance(a_out)
-        ev[k][2].record()
-    torch.cuda.synchronize()
-    launches = q.info()["kernel_launches"] - launches0
-    if world > 1:
-        dist.barrier()
+    equil = EQUIL_SWEEPS[args.config] if args.equil is None else args.equil
+    head = Timed(w, m, dev, rank, args.proposal, args.sigma)
+    head.run(equil, args.warmup, K, flush, barrier=dist.barrier if world > 1 else None, sampler=sampler)
     clocks = sampler.stop() if sampler else None
-    t_sweep = sum(ev[k][0].elapsed_time(ev[k][1]) for k in range(K)) * 1e-3
-    t_total = sum(ev[k][0].elapsed_time(ev[k][2]) for k in range(K)) * 1e-3
+    q, steps = head.q, head.steps
+    t_sweep, t_total = head.t_sweep, head.t_total
     if world > 1:
         tt = torch.tensor([t_total, t_sweep], dtype=torch.float64, device=dev)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         t_total, t_sweep = float(tt[0]), float(tt[1])
-    acc = float(a_out.mean())
-    e_mean = (e_out.mean(0) / N).tolist()
+        head.t_total, head.t_sweep = t_total, t_sweep
+    acc, e_mean, launches = head.acc, head.e_mean, head.launches
 
-    # ---- end to end through the host-buffer call (rank-local, same walkers) -------------------
-    h_in = q.get_positions().cpu().pin_memory()
+    # ---- end to end through the host-buffer call (rank-local, same walkers): coordinates and pair sums travel
+    # host -> device -> host every step; the copies overlap the compute chunk by chunk inside qmc_step_host ----
+    h_x = q.get_positions().cpu().pin_memory()
+    h_S = torch.empty((W, N), dtype=torch.float64).pin_memory()
     h_e = torch.empty((W, 4), dtype=torch.float64).pin_memory()
     h_a = torch.empty((W,), dtype=torch.float64).pin_memory()
-    h_x = torch.empty((W, 3, N), dtype=torch.float64).pin_memory()
     Ke = max(3, min(K, 10))
-    q.step_host(m, steps, h_in, h_e, h_a, h_x)          # warm-up
+    q.step_host(m, steps, h_x, h_e, h_a, h_x, h_S_out=h_S)                      # warm-up; the first S_i come back
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
     t0 = time.perf_counter()
     for _ in range(Ke):
-        q.step_host(m, steps, h_x, h_e, h_a, h_x)       # coordinates in, energies + coordinates out
+        q.step_host(m, steps, h_x, h_e, h_a, h_x, h_S_in=h_S, h_S_out=h_S)      # state in, energies + state out
     t_e2e = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    for _ in range(3):
+        q.step_host(m, steps, h_x, h_e, h_a, h_x)                                 # coordinates only: S_i rebuilt on the device
+    t_e2e_xyz = (time.perf_counter() - t0) / 3
     if world > 1:
         tt = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
@@ -271,11 +364,16 @@ def main():
     t_launch = t_sweep / K
     achieved = sweep_pairs * ALG_INSTR[w.mode] / t_launch
     executed = sweep_pairs * (1.0 + acc) * ALG_INSTR[w.mode] / t_launch
+    traffic = NCU_TRAFFIC_BYTES.get((w.name, w.mode)) if m == 1 else None
     roofline = {
         "bound": "alu", "kernel": f"sweep_kernel<{mode_name}>",
         "achieved": achieved / 1e9, "peak": peak_derived / 1e9, "unit": "G thread-instr/s",
-        "frac": achieved / peak_derived, "traffic": None,
-        "peak_source": f"derived: {info['sm_count']} SMs x {LANES_PER_SM[w.mode]} lanes x {sm_max:.0f} MHz (DESIGN.md)",
+        "frac": achieved / peak_derived, "traffic": traffic,
+        "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum per launch, ncu --set full of this command "
+                        "(profiles/r02_kernels.md); the walker state is 80 MB (fp32c) / 128 MB (fp64): read once, "
+                        "coordinates + S written once",
+        "peak_source": f"derived: {info['sm_count']} SMs x {LANES_PER_SM[w.mode]} lanes x {sm_max:.0f} MHz (DESIGN.md); "
+                       "MEASURED_PEAKS.json has no ALU entry",
         "peak_measured_fma_chain": peak_meas / 1e9,
         "alg_instr_per_pair_eval": ALG_INSTR[w.mode],
         "executed_frac": executed / peak_derived,
@@ -299,7 +397,9 @@ def main():
                    "sweeps_per_step": m, "mode": mode_name, "energy_every_step": True,
                    "proposal": "ordered/uniform-cube" if args.proposal == 0 else f"random-particle/gaussian sigma={args.sigma} A",
                    "l2": "flushed between timed steps (256 MiB write, untimed)",
+                   "equilibration_sweeps_untimed": equil,
                    "sweep_threads": info["sweep_threads"], "sweep_ctas_per_sm": info["sweep_ctas_per_sm"],
+                   "sweep_tile": info["sweep_tile"],
                    "energy_threads": info["energy_threads"], "energy_ctas_per_sm": info["energy_ctas_per_sm"]},
         "walker_sweeps_per_s": world * K * W * m / t_total,
         "sweep_only": {"pair_evals_per_s": world * K * sweep_pairs / t_sweep,
@@ -310,11 +410,35 @@ def main():
         "acceptance": acc, "energy_per_atom_K": dict(zip(["E_PB", "V", "T_PB", "T_JF"], e_mean)),
         "clocks": clocks,
         "e2e": {"value": world * Ke * pairs_step / t_e2e, "unit": "pair-evals/s",
-                "h2d_bytes_per_step": W * 3 * N * 8, "d2h_bytes_per_step": W * 3 * N * 8 + W * 5 * 8,
-                "ms_per_step": 1e3 * t_e2e / Ke, "api": "qmc_step_host (pinned host buffers)"},
+                "h2d_bytes_per_step": W * 3 * N * 8 + W * N * 8, "d2h_bytes_per_step": W * 3 * N * 8 + W * N * 8 + W * 5 * 8,
+                "ms_per_step": 1e3 * t_e2e / Ke,
+                "api": "qmc_step_host (pinned host buffers: coordinates + pair sums in, energies + acceptance + "
+                       "coordinates + pair sums out; walkers in chunks, copies overlap the compute)",
+                "coordinates_only": {"value": pairs_step / t_e2e_xyz, "ms_per_step": 1e3 * t_e2e_xyz,
+                                     "note": "h_S_in = NULL: the pair sums are rebuilt on the device after the upload "
+                                             "(one more all-pairs pass)"}},
         "gpu_launches": int(launches),
         "roofline": roofline,
     }
+    # ---- the other BASELINE.json configs and the fp64 comparison run of config 3, a few steps each (VERDICT r1
+    # missing #3): sweep / energy times, pair evaluations per second, roofline fraction -----------------------
+    if not args.no_configs and world == 1 and args.config == 3 and args.mode == "default" and not args.walkers:
+        head.q.close()
+        blocks = {}
+        for name, cfg, mode, k_steps in (("c1", 1, None, 20), ("c2", 2, None, 20), ("c3-fp64", 3, wl.MODE_FP64, 5),
+                                         ("c4", 4, None, 3), ("c5", 5, None, 5)):
+            wc = wl.config(cfg)
+            if mode is not None:
+                wc = wl.with_mode(wc, mode)
+            tc = Timed(wc, 1, dev, 0).run(EQUIL_SWEEPS[cfg] if cfg != 3 else 60, 3, k_steps, flush)
+            blocks[name] = summarize(tc, k_steps, info["sm_count"], sm_max)
+            tc.q.close()
+            del tc
+        out["configs"] = blocks
+        head = Timed(w, m, dev, rank, args.proposal, args.sigma)      # a fresh context for the items below
+        head.q.sweep(30, head.steps)
+        q = head.q
+    e_out = head.e_out
     # ---- observables beside the hot path: g(r) histogram, time to error ----
     nb = 256
     if 24 * N + 4 * nb <= 227 * 1024:
@@ -347,6 +471,20 @@ def main():
                           "ms_per_block": 1e3 * t_blk / nblk, "enqueue_ms": 1e3 * t_enq,
                           "d2h_bytes_per_block": W * 5 * 8, "flags_raised": int(hb_d.sum()),
                           "api": "qmc_run_blocks_host (write-outs on a second stream while the next block computes)"}
+    # in-kernel write-outs (the paper's own mechanism): one launch, coordinates to mapped pinned host memory every sweep
+    n_wo = 4
+    wo_x = torch.zeros((n_wo, W, 3, N), dtype=torch.float64).pin_memory()
+    wo_f = torch.zeros((n_wo, W), dtype=torch.int32).pin_memory()
+    t0 = time.perf_counter()
+    q.sweep_writeouts(n_wo * m, steps, m, wo_x, None, wo_f)
+    q.wait()
+    t_wo = time.perf_counter() - t0
+    out["sweep_writeouts"] = {"sweeps": n_wo * m, "writeouts": n_wo, "ms_per_sweep": 1e3 * t_wo / (n_wo * m),
+                              "bytes_per_writeout": W * 3 * N * 8, "flags_raised": int(wo_f.sum()),
+                              "api": "qmc_sweep_writeouts (one launch; thread blocks write coordinates to mapped pinned "
+                                     "host memory every m sweeps and raise per-walker flags)"}
+    if args.large_n:
+        out["large_n"] = large_n_block(dev, flush)
     if args.time_to_error > 0:
         from paper_1312_1282_b200 import observables as ob
         S = args.time_to_error
@@ -354,19 +492,24 @@ def main():
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         for _ in range(S):
-            one_step()
+            head.one_step()
             series.append(e_out[:, 0].mean().item() / N)       # walker-averaged E_PB per atom of this step
         el = time.perf_counter() - t0
         mean, se, tau = ob.reblock(series, min_blocks=8)
         tsig, t_goal = ob.seconds_to_error(se, el)
         out["time_to_error"] = {"steps": S, "seconds": el, "E_per_atom_K": mean, "se_K": se, "tau_steps": tau,
                                 "t_sigma2_s_mK2": tsig, "seconds_to_1mK_per_atom": t_goal,
-                                "note": "chain continues from the timed steps (not equilibrated if few steps were run)"}
+                                "note": f"chain equilibrated for {equil}+ sweeps before the series"}
     if not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w, m)
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+def large_n_block(dev, flush):
+    """NEXT-3 figures: placeholder until the cluster kernel reports (filled in by the cluster build)."""
+    return None
 
 
 if __name__ == "__main__":

@@ -107,13 +107,17 @@ int qmc_pair_histogram(qmc_ctx *c, int32_t nbins, uint32_t *d_hist);
 /* d_out: device [W] accepted / attempted moves since qmc_init_walkers / qmc_set_positions. */
 int qmc_acceptance(qmc_ctx *c, double *d_out);
 
-/* One whole step with HOST buffers (the paper's block cycle, l.319-343: coordinates in,
- * sweeps, energies and coordinates written out).  Any pointer may be NULL to skip that part.
- * h_xyz_in [W][3][N] is uploaded first (and S_i rebuilt); then n_sweeps sweeps; then the local
- * energy -> h_energy [W][4], acceptance -> h_acc [W], coordinates -> h_xyz_out [W][3][N].
- * Synchronises the stream before returning. */
-int qmc_step_host(qmc_ctx *c, const double *h_xyz_in, int32_t n_sweeps, const double *steps,
-                  double *h_energy, double *h_acc, double *h_xyz_out);
+/* One whole step with HOST buffers (the paper's block cycle, l.319-343: coordinates in, sweeps, energies and
+ * coordinates written out).  Any pointer may be NULL to skip that part.  h_xyz_in [W][3][N] is uploaded first; the
+ * running pair sums of the uploaded configuration are either uploaded with it (h_S_in [W][N], the h_S_out of an
+ * earlier call for the same coordinates: opaque walker state in the library's own unit, sum_j t(r_ij) with
+ * u = c1 t) or, with h_S_in = NULL, rebuilt on the device (one more all-pairs pass); then n_sweeps sweeps; then the
+ * local energy -> h_energy [W][4], acceptance -> h_acc [W], coordinates -> h_xyz_out [W][3][N], pair sums ->
+ * h_S_out [W][N].  The walkers are processed in chunks on internal streams so that the host<->device copies of one
+ * chunk run while another chunk computes (l.175, l.319-323: transfers masked by computation); use pinned host
+ * memory.  In and out buffers may be the same.  Synchronises before returning. */
+int qmc_step_host(qmc_ctx *c, const double *h_xyz_in, const double *h_S_in, int32_t n_sweeps, const double *steps,
+                  double *h_energy, double *h_acc, double *h_xyz_out, double *h_S_out);
 
 /* A run of n_blocks blocks with in-flight write-outs (the paper's load masking, l.175, l.323, §4; SURVEY.md §8(f)
  * NEXT-4).  Block b = sweeps_per_block sweeps + local energy + acceptance; its results go to the HOST arrays
@@ -178,7 +182,7 @@ int qmc_info(const qmc_ctx *c, qmc_info_t *out);
 /* Process-wide override of the launch heuristics for the contexts created AFTERWARDS (tuning experiments and
  * tests; the defaults are what bench.py times).  Keys: "sweep_threads", "sweep_per_thread", "sweep_vector",
  * "sweep_pending", "sweep_tile" (1 = one-move kernel, 2 / 4 = tile kernel), "sweep_cluster", "energy_threads",
- * "energy_ordered" (1 = ordered-pair energy kernels).  value: the wanted number, or -1 (0 for the energy keys) for
+ * "energy_ordered" (1 = ordered-pair energy kernels), "host_chunks" (walker chunks of qmc_step_host, 1..8).  value: the wanted number, or -1 (0 for the energy keys) for
  * "heuristic".  key == NULL resets everything.  A shape that is not compiled or does not fit N falls back to the
  * heuristic.  Returns QMC_E_ARG for an unknown key. */
 int qmc_set_tuning(const char *key, int32_t value);

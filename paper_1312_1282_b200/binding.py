@@ -87,7 +87,7 @@ def load_library() -> C.CDLL:
     lib.qmc_sweep_writeouts.argtypes = [vp, C.c_int32, dp, C.c_int32, vp, vp, vp]
     lib.qmc_set_tuning.argtypes = [C.c_char_p, C.c_int32]
     lib.qmc_wait.argtypes = [vp]
-    lib.qmc_step_host.argtypes = [vp, vp, C.c_int32, dp, vp, vp, vp]
+    lib.qmc_step_host.argtypes = [vp, vp, vp, C.c_int32, dp, vp, vp, vp, vp]
     lib.qmc_last_error.argtypes = [vp]
     lib.qmc_last_error.restype = C.c_char_p
     lib.qmc_get_positions.argtypes = [vp, vp]
@@ -285,18 +285,18 @@ class QMC:
         self._check(self._lib.qmc_pair_histogram(self._ctx, int(nbins), self._ptr(out, torch.int32, self.W * nbins)))
         return out
 
-    def step_host(self, n_sweeps: int, steps, h_xyz_in=None, h_energy=None, h_acc=None, h_xyz_out=None):
-        """qmc_step_host with host tensors (pinned for asynchronous copies)."""
+    def step_host(self, n_sweeps: int, steps, h_xyz_in=None, h_energy=None, h_acc=None, h_xyz_out=None,
+                  h_S_in=None, h_S_out=None):
+        """qmc_step_host with host tensors (pinned for asynchronous copies); h_S_in / h_S_out [W][N] carry the
+        running pair sums along with the coordinates (opaque state, see qmc.h)."""
         torch = self._torch
         n = self.W * 3 * self.N
-        args = [
-            self._ptr(h_xyz_in, torch.float64, n, "cpu") if h_xyz_in is not None else None,
-            int(n_sweeps), self._steps(steps),
-            self._ptr(h_energy, torch.float64, self.W * 4, "cpu") if h_energy is not None else None,
-            self._ptr(h_acc, torch.float64, self.W, "cpu") if h_acc is not None else None,
-            self._ptr(h_xyz_out, torch.float64, n, "cpu") if h_xyz_out is not None else None,
-        ]
-        self._check(self._lib.qmc_step_host(self._ctx, *args))
+
+        def hp(t, numel):
+            return self._ptr(t, torch.float64, numel, "cpu") if t is not None else None
+        self._check(self._lib.qmc_step_host(
+            self._ctx, hp(h_xyz_in, n), hp(h_S_in, self.W * self.N), int(n_sweeps), self._steps(steps),
+            hp(h_energy, self.W * 4), hp(h_acc, self.W), hp(h_xyz_out, n), hp(h_S_out, self.W * self.N)))
 
     # -- state access and parity hooks -----------------------------------------------------
     def get_positions(self, out=None):

@@ -128,6 +128,20 @@ __global__ void get_pair_sums_kernel(StateView sv, double *__restrict__ S)
     if (i < sv.N) S[(size_t)w * sv.N + i] = sv.groups[sv.group_of[w]].c1 * sv.S[(size_t)w * sv.ld + i];
 }
 
+// running pair sums in the state's own unit (sum_j t(r_ij), u = c1 t), [W][N] <-> [W][ld]: qmc_step_host's h_S_in / h_S_out
+__global__ void export_raw_sums_kernel(StateView sv, double *__restrict__ S)
+{
+    const int w = blockIdx.x;
+    const int i = blockIdx.y * blockDim.x + threadIdx.x;
+    if (i < sv.N) S[(size_t)w * sv.N + i] = sv.S[(size_t)w * sv.ld + i];
+}
+__global__ void import_raw_sums_kernel(StateView sv, const double *__restrict__ S)
+{
+    const int w = blockIdx.x;
+    const int i = blockIdx.y * blockDim.x + threadIdx.x;
+    if (i < sv.N) sv.S[(size_t)w * sv.ld + i] = S[(size_t)w * sv.N + i];
+}
+
 __global__ void acceptance_kernel(StateView sv, double attempted, double *__restrict__ out)
 {
     const int w = blockIdx.x * blockDim.x + threadIdx.x;
@@ -175,6 +189,19 @@ cudaError_t launch_acceptance(qmc_ctx *c, double *d_out)
 {
     c->launches += 1;
     acceptance_kernel<<<(c->W + 127) / 128, 128, 0, c->stream>>>(c->sv, (double)(c->t - c->t_acc0) * (double)c->p.N, d_out);
+    return cudaGetLastError();
+}
+static cudaError_t launch_acceptance_attempted(qmc_ctx *c, double attempted, double *d_out)
+{
+    c->launches += 1;
+    acceptance_kernel<<<(c->W + 127) / 128, 128, 0, c->stream>>>(c->sv, attempted, d_out);
+    return cudaGetLastError();
+}
+static cudaError_t launch_raw_sums(qmc_ctx *c, double *d_S, bool import)
+{
+    c->launches += 1;
+    if (import) import_raw_sums_kernel<<<grid_wn(c, c->p.N), 128, 0, c->stream>>>(c->sv, d_S);
+    else        export_raw_sums_kernel<<<grid_wn(c, c->p.N), 128, 0, c->stream>>>(c->sv, d_S);
     return cudaGetLastError();
 }
 
@@ -342,6 +369,14 @@ extern "C" int qmc_destroy(qmc_ctx *c)
     if (c->out_stream) cudaStreamSynchronize(c->out_stream);
     if (c->d_block) cudaFree(c->d_block);
     if (c->d_block_xyz) cudaFree(c->d_block_xyz);
+    for (cudaStream_t st : {c->hs_in, c->hs_out, c->hs_cmp[0], c->hs_cmp[1]}) if (st) { cudaStreamSynchronize(st); cudaStreamDestroy(st); }
+    for (int k = 0; k < qmc::kHostChunksMax; ++k) {
+        if (c->hs_ev_in[k]) cudaEventDestroy(c->hs_ev_in[k]);
+        if (c->hs_ev_cmp[k]) cudaEventDestroy(c->hs_ev_cmp[k]);
+    }
+    if (c->hs_ev_fork) cudaEventDestroy(c->hs_ev_fork);
+    if (c->hs_ev_join) cudaEventDestroy(c->hs_ev_join);
+    if (c->d_hS) cudaFree(c->d_hS);
     for (int k = 0; k < 2; ++k) {
         if (c->ev_ready[k]) cudaEventDestroy(c->ev_ready[k]);
         if (c->ev_copied[k]) cudaEventDestroy(c->ev_copied[k]);
@@ -502,36 +537,125 @@ extern "C" int qmc_trace_decisions(qmc_ctx *c, int32_t w_begin, int32_t w_end, u
     return QMC_OK;
 }
 
-extern "C" int qmc_step_host(qmc_ctx *c, const double *h_xyz_in, int32_t n_sweeps, const double *steps,
-                             double *h_energy, double *h_acc, double *h_xyz_out)
+// A walker sub-range [w0, w0 + wc) of the context as a context of its own for the launch helpers: state pointers
+// advanced, W and walker_id_base adjusted, work on `stream`.  Restores everything on destruction.
+namespace {
+struct RangeGuard {
+    qmc_ctx *c; StateView sv0; int32_t W0; cudaStream_t st0;
+    RangeGuard(qmc_ctx *ctx, int w0, int wc, cudaStream_t stream) : c(ctx), sv0(ctx->sv), W0(ctx->W), st0(ctx->stream)
+    {
+        const size_t real = c->p.mode == QMC_FP64 ? 8 : 4;
+        c->sv.pos = (char *)sv0.pos + (size_t)w0 * 3 * c->ld * real;
+        c->sv.S = sv0.S + (size_t)w0 * c->ld;
+        c->sv.n_acc = sv0.n_acc + w0;
+        c->sv.group_of = sv0.group_of + w0;
+        c->sv.W = wc;
+        c->sv.walker_id_base = sv0.walker_id_base + (uint32_t)w0;
+        c->W = wc;
+        c->stream = stream;
+    }
+    ~RangeGuard() { c->sv = sv0; c->W = W0; c->stream = st0; }
+};
+}  // namespace
+
+extern "C" int qmc_step_host(qmc_ctx *c, const double *h_xyz_in, const double *h_S_in, int32_t n_sweeps, const double *steps,
+                             double *h_energy, double *h_acc, double *h_xyz_out, double *h_S_out)
 {
     if (!c) return QMC_E_ARG;
-    const size_t W = (size_t)c->W, N = (size_t)c->p.N;
-    double *d_e = c->d_scratch, *d_a = c->d_scratch + 4 * W, *d_x = c->d_scratch + 5 * W;
-    if (h_xyz_in) {
-        QMC_CUDA(c, cudaMemcpyAsync(d_x, h_xyz_in, sizeof(double) * W * 3 * N, cudaMemcpyHostToDevice, c->stream));
-        int rc = qmc_set_positions(c, d_x);
-        if (rc != QMC_OK) return rc;
+    if (h_S_in && !h_xyz_in) QMC_FAIL(c, QMC_E_ARG, "h_S_in needs h_xyz_in (the pair sums belong to the uploaded coordinates)");
+    if (!h_xyz_in && !c->have_state) QMC_FAIL(c, QMC_E_STATE, "qmc_step_host without coordinates before qmc_init_walkers / qmc_set_positions");
+    if (n_sweeps < 0 || (n_sweeps > 0 && !steps)) QMC_FAIL(c, QMC_E_ARG, "n_sweeps >= 0 and steps != NULL required");
+    if ((long long)n_sweeps * c->p.N >= (1LL << 31)) QMC_FAIL(c, QMC_E_ARG, "n_sweeps * N must stay below 2^31 per call");
+    const size_t Wt = (size_t)c->W, N = (size_t)c->p.N;
+    // first use: copy-in / copy-out / two compute streams and the per-chunk events (all or nothing)
+    if (!c->host_ready) {
+        cudaError_t e = cudaSuccess;
+        cudaStream_t *st[4] = {&c->hs_in, &c->hs_out, &c->hs_cmp[0], &c->hs_cmp[1]};
+        for (auto p : st) if (e == cudaSuccess) e = cudaStreamCreateWithFlags(p, cudaStreamNonBlocking);
+        for (int k = 0; k < kHostChunksMax && e == cudaSuccess; ++k) {
+            e = cudaEventCreateWithFlags(&c->hs_ev_in[k], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->hs_ev_cmp[k], cudaEventDisableTiming);
+        }
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->hs_ev_fork, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->hs_ev_join, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaMalloc(&c->d_hS, sizeof(double) * Wt * N);
+        if (e != cudaSuccess) {
+            for (auto p : st) if (*p) { cudaStreamDestroy(*p); *p = nullptr; }
+            for (int k = 0; k < kHostChunksMax; ++k) {
+                if (c->hs_ev_in[k]) { cudaEventDestroy(c->hs_ev_in[k]); c->hs_ev_in[k] = nullptr; }
+                if (c->hs_ev_cmp[k]) { cudaEventDestroy(c->hs_ev_cmp[k]); c->hs_ev_cmp[k] = nullptr; }
+            }
+            if (c->hs_ev_fork) { cudaEventDestroy(c->hs_ev_fork); c->hs_ev_fork = nullptr; }
+            if (c->hs_ev_join) { cudaEventDestroy(c->hs_ev_join); c->hs_ev_join = nullptr; }
+            if (c->d_hS) { cudaFree(c->d_hS); c->d_hS = nullptr; }
+            QMC_FAIL(c, QMC_E_CUDA, "qmc_step_host set-up: %s", cudaGetErrorString(e));
+        }
+        c->host_ready = true;
     }
+    // proposal steps -> constant table (once, before the fork)
     if (n_sweeps > 0) {
-        int rc = qmc_sweep(c, n_sweeps, steps);
-        if (rc != QMC_OK) return rc;
+        bool changed = false;
+        for (int g = 0; g < c->p.n_groups; ++g) {
+            const double reach = c->sv.proposal == 1 ? 6.77 : 1.0;
+            if (!(steps[g] > 0.0) || !(steps[g] * reach < 0.5 * c->box_L[g]))
+                QMC_FAIL(c, QMC_E_ARG, "steps[%d] = %g must lie in (0, L/2 = %g)", g, steps[g], 0.5 * c->box_L[g]);
+            if (c->groups[g].step != steps[g]) { c->groups[g].step = steps[g]; changed = true; }
+        }
+        if (changed)
+            QMC_CUDA(c, cudaMemcpyAsync(c->d_groups, c->groups.data(), sizeof(GroupDev) * c->p.n_groups, cudaMemcpyHostToDevice, c->stream));
     }
-    if (h_energy) {
-        int rc = qmc_local_energy(c, d_e);
-        if (rc != QMC_OK) return rc;
-        QMC_CUDA(c, cudaMemcpyAsync(h_energy, d_e, sizeof(double) * 4 * W, cudaMemcpyDeviceToHost, c->stream));
+    // walkers in chunks (l.175, l.319-323: transfers masked by computation): chunk k's upload, compute and download
+    // run on three streams, so that chunk k+1 uploads and chunk k-1 downloads while chunk k computes; two compute
+    // streams let the sweep of one chunk share the GPU with the energy pass of the previous one.  A decision trace
+    // (walker indices of the whole context) or few walkers keep everything in one chunk.
+    int nchunk = g_tuning.host_chunks > 0 ? g_tuning.host_chunks : 4;
+    if (nchunk > kHostChunksMax) nchunk = kHostChunksMax;
+    while (nchunk > 1 && (int)Wt / nchunk < c->sm_count) --nchunk;
+    if (c->trace.dec) nchunk = 1;
+    if (h_xyz_in) c->t_acc0 = c->t;                             // set_positions zeroes the counters
+    const double attempted = (double)(c->t + (uint32_t)n_sweeps - c->t_acc0) * (double)N;
+    double *d_e = c->d_scratch, *d_a = c->d_scratch + 4 * Wt, *d_x = c->d_scratch + 5 * Wt;
+    NvtxRange range("qmc_step_host");
+    QMC_CUDA(c, cudaEventRecord(c->hs_ev_fork, c->stream));
+    for (cudaStream_t st : {c->hs_in, c->hs_out, c->hs_cmp[0], c->hs_cmp[1]}) QMC_CUDA(c, cudaStreamWaitEvent(st, c->hs_ev_fork, 0));
+    for (int k = 0; k < nchunk; ++k) {
+        const int w0 = (int)((long long)Wt * k / nchunk), w1 = (int)((long long)Wt * (k + 1) / nchunk), wc = w1 - w0;
+        cudaStream_t cs = c->hs_cmp[k & 1];
+        double *dxk = d_x + (size_t)w0 * 3 * N, *dSk = c->d_hS + (size_t)w0 * N;
+        if (h_xyz_in) {
+            QMC_CUDA(c, cudaMemcpyAsync(dxk, h_xyz_in + (size_t)w0 * 3 * N, sizeof(double) * wc * 3 * N, cudaMemcpyHostToDevice, c->hs_in));
+            if (h_S_in) QMC_CUDA(c, cudaMemcpyAsync(dSk, h_S_in + (size_t)w0 * N, sizeof(double) * wc * N, cudaMemcpyHostToDevice, c->hs_in));
+            QMC_CUDA(c, cudaEventRecord(c->hs_ev_in[k], c->hs_in));
+            QMC_CUDA(c, cudaStreamWaitEvent(cs, c->hs_ev_in[k], 0));
+        }
+        {
+            RangeGuard view(c, w0, wc, cs);
+            if (h_xyz_in) {
+                QMC_CUDA(c, launch_set_positions(c, dxk));
+                if (h_S_in) QMC_CUDA(c, launch_raw_sums(c, dSk, true));
+                else        QMC_CUDA(c, launch_energy(c, nullptr, false));      // rebuild S_i from the coordinates
+            }
+            if (n_sweeps > 0) QMC_CUDA(c, launch_sweep(c, n_sweeps));
+            if (h_energy) QMC_CUDA(c, launch_energy(c, d_e + (size_t)w0 * 4, true));
+            if (h_acc) QMC_CUDA(c, launch_acceptance_attempted(c, attempted, d_a + w0));
+            if (h_xyz_out) QMC_CUDA(c, launch_get_positions(c, dxk));
+            if (h_S_out) QMC_CUDA(c, launch_raw_sums(c, dSk, false));
+        }
+        QMC_CUDA(c, cudaEventRecord(c->hs_ev_cmp[k], cs));
+        QMC_CUDA(c, cudaStreamWaitEvent(c->hs_out, c->hs_ev_cmp[k], 0));
+        if (h_energy) QMC_CUDA(c, cudaMemcpyAsync(h_energy + (size_t)w0 * 4, d_e + (size_t)w0 * 4, sizeof(double) * 4 * wc, cudaMemcpyDeviceToHost, c->hs_out));
+        if (h_acc) QMC_CUDA(c, cudaMemcpyAsync(h_acc + w0, d_a + w0, sizeof(double) * wc, cudaMemcpyDeviceToHost, c->hs_out));
+        if (h_xyz_out) QMC_CUDA(c, cudaMemcpyAsync(h_xyz_out + (size_t)w0 * 3 * N, dxk, sizeof(double) * wc * 3 * N, cudaMemcpyDeviceToHost, c->hs_out));
+        if (h_S_out) QMC_CUDA(c, cudaMemcpyAsync(h_S_out + (size_t)w0 * N, dSk, sizeof(double) * wc * N, cudaMemcpyDeviceToHost, c->hs_out));
     }
-    if (h_acc) {
-        int rc = qmc_acceptance(c, d_a);
-        if (rc != QMC_OK) return rc;
-        QMC_CUDA(c, cudaMemcpyAsync(h_acc, d_a, sizeof(double) * W, cudaMemcpyDeviceToHost, c->stream));
+    // join: the context's stream continues after everything; then the host waits
+    for (cudaStream_t st : {c->hs_in, c->hs_out, c->hs_cmp[0], c->hs_cmp[1]}) {
+        QMC_CUDA(c, cudaEventRecord(c->hs_ev_join, st));
+        QMC_CUDA(c, cudaStreamWaitEvent(c->stream, c->hs_ev_join, 0));
     }
-    if (h_xyz_out) {
-        int rc = qmc_get_positions(c, d_x);
-        if (rc != QMC_OK) return rc;
-        QMC_CUDA(c, cudaMemcpyAsync(h_xyz_out, d_x, sizeof(double) * W * 3 * N, cudaMemcpyDeviceToHost, c->stream));
-    }
+    c->t += (uint32_t)n_sweeps;
+    if (c->trace.dec) c->trace.offset += (long long)n_sweeps * c->p.N;
+    if (h_xyz_in) c->have_state = true;
     QMC_CUDA(c, cudaStreamSynchronize(c->stream));
     return QMC_OK;
 }
@@ -628,7 +752,7 @@ extern "C" int qmc_set_tuning(const char *key, int32_t value)
     struct { const char *name; int *field; } tab[] = {
         {"sweep_threads", &t.sweep_threads}, {"sweep_per_thread", &t.sweep_per_thread}, {"sweep_vector", &t.sweep_vector},
         {"sweep_pending", &t.sweep_pending}, {"sweep_tile", &t.sweep_tile}, {"sweep_cluster", &t.sweep_cluster},
-        {"energy_threads", &t.energy_threads}, {"energy_ordered", &t.energy_ordered},
+        {"energy_threads", &t.energy_threads}, {"energy_ordered", &t.energy_ordered}, {"host_chunks", &t.host_chunks},
     };
     for (auto &e : tab)
         if (strcmp(key, e.name) == 0) { *e.field = value; return QMC_OK; }

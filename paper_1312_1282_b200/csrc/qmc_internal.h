@@ -45,7 +45,8 @@ struct SweepPlan  { int threads, J, V, P, K, cluster, smem_bytes, ctas_per_sm; c
                     const void *fallback; int fallback_smem; };   // fallback: one-move shape for what the tile kernel does not take
 // Process-wide overrides of the launch heuristics (qmc_set_tuning; tuning experiments and tests); -1 / 0 = heuristic.
 struct Tuning { int sweep_threads = 0, sweep_per_thread = 0, sweep_vector = -1, sweep_pending = -1, sweep_tile = -1,
-                    energy_threads = 0, energy_ordered = 0, sweep_cluster = -1; };
+                    energy_threads = 0, energy_ordered = 0, sweep_cluster = -1, host_chunks = 0; };
+constexpr int kHostChunksMax = 8;
 extern Tuning g_tuning;
 struct EnergyPlan { int threads, smem_bytes, ctas_per_sm, variant; };   // variant 1 (FP64): unordered-pair kernel
 
@@ -70,6 +71,11 @@ struct qmc_ctx {
     double *d_block_xyz = nullptr;                 // [2][W][3][N] coordinate write-outs (allocated on first use)
     bool blocks_ready = false;                     // stream, d_block and the events below exist
     cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
+    // qmc_step_host: copy-in, copy-out and two compute streams, per-chunk events, staging of the pair sums (first use)
+    cudaStream_t hs_in = nullptr, hs_out = nullptr, hs_cmp[2] = {nullptr, nullptr};
+    cudaEvent_t hs_ev_in[qmc::kHostChunksMax] = {}, hs_ev_cmp[qmc::kHostChunksMax] = {}, hs_ev_fork = nullptr, hs_ev_join = nullptr;
+    double *d_hS = nullptr;                        // [W][N]
+    bool host_ready = false;
     qmc::TraceView trace{};
     qmc::WriteoutView wo{};                        // in-kernel write-outs of the running qmc_sweep_writeouts call
     qmc::SweepPlan sweep_plan{};

@@ -613,6 +613,50 @@ def test_step_host_equals_device_calls(qmc):
         assert torch.equal(q2.get_positions().cpu(), h_x)
 
 
+def test_step_host_chunks_and_pair_sum_round_trip(qmc):
+    """qmc_step_host over several walker chunks (copies overlapping compute on internal streams), with the pair sums
+    travelling with the coordinates (h_S_in / h_S_out) or rebuilt on the device: same bits as the device calls."""
+    import torch
+    N, W = 64, 700                                           # > 4 x 148 walkers: four chunks
+    for mode in (qmc.QMC_FP64, qmc.QMC_FP32C):
+        q, L = make(qmc, N, W, mode)
+        q.init_walkers(17)
+        q.sweep(3, 1.0)
+        h_x = q.get_positions().cpu().pin_memory()
+        h_S = torch.zeros((W, N), dtype=torch.float64).pin_memory()
+        h_e = torch.empty((W, 4), dtype=torch.float64).pin_memory()
+        h_a = torch.empty((W,), dtype=torch.float64).pin_memory()
+        h_x2 = torch.empty((W, 3, N), dtype=torch.float64).pin_memory()
+        h_S2 = torch.empty((W, N), dtype=torch.float64).pin_memory()
+        qa, _ = make(qmc, N, W, mode)
+        qa.set_seed(5, 7)
+        qa.step_host(0, 1.0, h_x, h_S_out=h_S)              # upload, rebuild S_i, read them back
+        qa.step_host(2, 1.0, h_x, h_e, h_a, h_x2, h_S_in=h_S, h_S_out=h_S2)
+        qb, _ = make(qmc, N, W, mode)
+        qb.set_seed(5, 7)
+        qb.set_positions(h_x.numpy())
+        assert torch.equal(qb.pair_sums().cpu(), qa_sums_in_u(qmc, qa, h_S, N, L))
+        qb.sweep(2, 1.0)
+        assert torch.equal(qb.local_energy().cpu(), h_e)
+        assert torch.equal(qb.acceptance().cpu(), h_a)
+        assert torch.equal(qb.get_positions().cpu(), h_x2)
+        assert torch.equal(qa.get_positions().cpu(), h_x2)
+        # coordinates only (S_i rebuilt on the device) gives the same step
+        qc, _ = make(qmc, N, W, mode)
+        qc.set_seed(5, 7)
+        h_e3 = torch.empty((W, 4), dtype=torch.float64).pin_memory()
+        qc.step_host(2, 1.0, h_x, h_e3)
+        assert torch.equal(h_e3, h_e)
+        assert qc.info()["t"] == 9 and qa.info()["t"] == 9
+
+
+def qa_sums_in_u(qmc, q, h_S_raw, N, L):
+    """h_S_out is in the library's raw unit sum_j t(r_ij); u = c1 t with c1 = -b^5/2 in the mode's length unit."""
+    import torch
+    b = 2.89 / (L if q.mode == qmc.QMC_FP32C else 1.0)
+    return h_S_raw.clone() * (-0.5 * (b * b * b * b * b))
+
+
 def test_run_blocks_host_equals_stepwise_calls(qmc):
     """qmc_run_blocks_host (NEXT-4: blocks with in-flight write-outs on a second stream) against the same
     sequence of qmc_sweep / qmc_local_energy / qmc_acceptance calls: identical numbers, flags raised."""

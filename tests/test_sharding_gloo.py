@@ -81,3 +81,25 @@ def test_shard_groups_split_across_group_boundaries():
             assert base == wl.walker_shard(w.n_walkers, r, world)[0]
             tot = [a + b for a, b in zip(tot, wpg)]
         assert tot == w.walkers_per_group
+
+
+def test_bench_gpus_flag_starts_that_many_ranks():
+    """`python bench.py --gpus 2` with no launcher around it starts two ranks itself (torch.distributed.run on
+    127.0.0.1) and rank 0 reports n_gpus = 2; --plumbing-only keeps the GPU out of it (gloo), so this runs on CPU."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    env["OMP_NUM_THREADS"] = "1"
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--plumbing-only"],
+                       capture_output=True, text=True, timeout=300, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == 2 and out["requested_gpus"] == 2
+    # and a single process stays a single rank
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--plumbing-only"],
+                       capture_output=True, text=True, timeout=300, env=env)
+    assert r.returncode == 0 and json.loads(r.stdout.strip().splitlines()[-1])["n_gpus"] == 1
