@@ -16,9 +16,9 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libqmc_b200.so")
 PROBE_LIB = os.path.join(HERE, "libqmc_probe_b200.so")      # measurement tool (include/qmc_probe.h), not the product
 PROBE_SRC = os.path.join(HERE, "probe", "qmc_probe.cu")
-SOURCES = ["qmc_api.cu", "qmc_sweep_plan.cu", "qmc_sweep_f32.cu", "qmc_sweep_f64.cu", "qmc_sweep_tile_f32.cu", "qmc_energy.cu",
+SOURCES = ["qmc_api.cu", "qmc_sweep_plan.cu", "qmc_sweep_f32.cu", "qmc_sweep_f64.cu", "qmc_sweep_tile_f32.cu", "qmc_sweep_cluster_f32.cu", "qmc_sweep_cluster_f64.cu", "qmc_energy.cu",
            "qmc_energy_f32.cu", "qmc_energy_f32s.cu", "qmc_energy_f64.cu", "qmc_observables.cu"]
-HEADERS = ["qmc_device.cuh", "qmc_internal.h", "qmc_sweep_impl.cuh", "qmc_sweep_tile.cuh", "qmc_f32c.cuh", "qmc_energy_f32_pair.cuh", os.path.join("..", "..", "include", "qmc.h")]
+HEADERS = ["qmc_device.cuh", "qmc_internal.h", "qmc_sweep_impl.cuh", "qmc_sweep_tile.cuh", "qmc_sweep_cluster.cuh", "qmc_f32c.cuh", "qmc_energy_f32_pair.cuh", os.path.join("..", "..", "include", "qmc.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]

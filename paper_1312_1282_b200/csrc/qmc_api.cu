@@ -272,6 +272,7 @@ extern "C" int qmc_create(const qmc_params *p, void *cuda_stream, void *d_state,
     long long W = 0;
     for (int g = 0; g < p->n_groups; ++g) W += p->walkers_per_group[g];
     c->W = (int32_t)W;
+    c->W_total = (int32_t)W;
 
 #define CREATE_FAIL(code, ...) do { snprintf(g_create_err, 512, __VA_ARGS__); qmc_destroy(c); return (code); } while (0)
 #define CREATE_CUDA(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) CREATE_FAIL(QMC_E_CUDA, "%s: %s", #expr, cudaGetErrorString(e__)); } while (0)
@@ -366,6 +367,8 @@ extern "C" int qmc_destroy(qmc_ctx *c)
     if (c->d_groups) cudaFree(c->d_groups);
     if (c->d_group_of) cudaFree(c->d_group_of);
     if (c->d_scratch) cudaFree(c->d_scratch);
+    if (c->d_enc) cudaFree(c->d_enc);
+    if (c->d_epart) cudaFree(c->d_epart);
     if (c->out_stream) cudaStreamSynchronize(c->out_stream);
     if (c->d_block) cudaFree(c->d_block);
     if (c->d_block_xyz) cudaFree(c->d_block_xyz);
@@ -437,6 +440,9 @@ extern "C" int qmc_sweep(qmc_ctx *c, int32_t n_sweeps, const double *steps)
     }
     if (changed)   // stream-ordered update of the small constant table (host mirror is ours, pageable copy is synchronous to the host)
         QMC_CUDA(c, cudaMemcpyAsync(c->d_groups, c->groups.data(), sizeof(GroupDev) * c->p.n_groups, cudaMemcpyHostToDevice, c->stream));
+    if (c->sweep_plan.cluster > 1 && (c->sv.proposal != 0 || c->wo.xyz != nullptr))
+        QMC_FAIL(c, QMC_E_ARG, "the cluster sweep kernel (N = %d on %d blocks per walker) takes proposal 0 and no in-kernel write-outs",
+                 c->p.N, c->sweep_plan.cluster);
     {
         NvtxRange r("qmc_sweep");
         QMC_CUDA(c, launch_sweep(c, n_sweeps));

@@ -187,9 +187,11 @@ static cudaError_t launch_e(qmc_ctx *c, double *d_out, bool energy)
 cudaError_t launch_energy(qmc_ctx *c, double *d_out, bool energy)
 {
     c->launches += 1;
-    if (c->p.mode != QMC_FP64)
+    if (c->p.mode != QMC_FP64) {
+        if (c->energy_plan.variant == 3) { c->launches -= 1; return launch_energy_f32g(c, d_out, energy); }   // counts its own launches
         return c->energy_plan.variant == 2 ? launch_energy_f32s(c, d_out, energy)    // qmc_energy_f32s.cu
                                            : launch_energy_f32(c, d_out, energy);    // qmc_energy_f32.cu
+    }
     if (c->energy_plan.variant == 1) return launch_energy_f64(c, d_out, energy);  // qmc_energy_f64.cu
     const int T = c->energy_plan.threads;
 #define X(TT) if (T == TT) return launch_e<double, TT>(c, d_out, energy);
@@ -201,12 +203,20 @@ cudaError_t launch_energy(qmc_ctx *c, double *d_out, bool energy)
 bool plan_energy(qmc_ctx *c, EnergyPlan *out)
 {
     out->variant = 0;
+    out->parts = 1;
     if (c->p.mode != QMC_FP64) {
-        if (!g_tuning.energy_ordered && plan_energy_f32s(c, out)) return true;
+        // one walker per block while that fills the GPU; the gridded kernel for few walkers of many atoms (a block
+        // per walker would leave SMs idle) and for N beyond one block's shared memory.
+        // qmc_set_tuning("energy_ordered"): 0 heuristic, 1 ordered pairs, 2 unordered pairs, 3 gridded.
+        const int want = g_tuning.energy_ordered;
+        const bool few = (long long)c->W * 2 < c->sm_count && c->p.N >= 1024;
+        if (want == 3 || (want == 0 && few)) return plan_energy_f32g(c, out);
+        if (want != 1 && plan_energy_f32s(c, out)) return true;
         out->variant = 0;
-        return plan_energy_f32(c, out);
+        if (plan_energy_f32(c, out)) return true;
+        return plan_energy_f32g(c, out);
     }
-    if (!g_tuning.energy_ordered && plan_energy_f64(c, out)) return true;
+    if (g_tuning.energy_ordered != 1 && plan_energy_f64(c, out)) return true;
     out->variant = 0;
     const int N = c->p.N;
     int T = 32;

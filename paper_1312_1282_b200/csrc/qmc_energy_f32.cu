@@ -38,7 +38,7 @@ struct Acc64 { double gx, gy, gz, lam, lamd, s, v; };   // lam: tiles above the 
 //   kSlow: per-pair selects (self pair, j >= N, V only for j > i); kV: evaluate the potential and the
 //   Laplacian term (both are symmetric in i,j and only their totals are needed: tiles below the diagonal skip them).
 // Sums kept here: gm = y^7 - z^6 y = (u'/r) / (5/2 b^5);  lt = 2 y^7 + 3 z^7 + z^6 y = -(u'' + 2u'/r) / (5 b^5).
-template <bool kEnergy, bool kV, bool kSlow>
+template <bool kEnergy, bool kV, bool kSlow, bool kGlobal = false>
 __device__ __forceinline__ void tile16(const int32_t *__restrict__ x, const int32_t *__restrict__ y, const int32_t *__restrict__ z,
                                        int j0, int i, int N, int32_t xi, int32_t yi, int32_t zi, const AzizF32 &E,
                                        int32_t zero, Acc64 &A, double &lam_acc, int &n_in)
@@ -47,9 +47,11 @@ __device__ __forceinline__ void tile16(const int32_t *__restrict__ x, const int3
     P.gx = P.gy = P.gz = P.lam = P.s = P.v = pk1(0.0f);
 #pragma unroll 1
     for (int g = 0; g < 4; ++g) {
-        const int4 X = *reinterpret_cast<const int4 *>(x + j0 + 4 * g);
-        const int4 Y = *reinterpret_cast<const int4 *>(y + j0 + 4 * g);
-        const int4 Z = *reinterpret_cast<const int4 *>(z + j0 + 4 * g);
+        // kGlobal: the coordinates stream from global memory through the read-only path (all lanes read the same
+        // address; the L1 serves the other warps of the block)
+        const int4 X = kGlobal ? __ldg(reinterpret_cast<const int4 *>(x + j0 + 4 * g)) : *reinterpret_cast<const int4 *>(x + j0 + 4 * g);
+        const int4 Y = kGlobal ? __ldg(reinterpret_cast<const int4 *>(y + j0 + 4 * g)) : *reinterpret_cast<const int4 *>(y + j0 + 4 * g);
+        const int4 Z = kGlobal ? __ldg(reinterpret_cast<const int4 *>(z + j0 + 4 * g)) : *reinterpret_cast<const int4 *>(z + j0 + 4 * g);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             const int ja = j0 + 4 * g + 2 * h, jb = ja + 1;
@@ -197,6 +199,120 @@ energy32_kernel(StateView sv, double Dk, double *__restrict__ out)
     }
 }
 
+// ---- gridded variant (energy_plan.variant 3): any N, and one walker on many SMs --------------
+// The walker's fixed-point coordinates sit in GLOBAL memory ([W][3][NP] int32, written by encode_kernel) and stream
+// through L1/L2 as broadcast 16-byte reads; block (w, part) of the grid takes the i-blocks A = part*nwarps + warp,
+// + nparts*nwarps, ... of walker w with the same tiles as energy32_kernel, writes their S_i and its three partial
+// sums; finalize_kernel adds the parts of a walker in a fixed order (deterministic) and forms the energies.
+__global__ void encode_kernel(StateView sv, int32_t *__restrict__ enc, int NP)
+{
+    const int w = blockIdx.x;
+    const int j = blockIdx.y * blockDim.x + threadIdx.x;
+    if (j >= NP) return;
+    const float *gpos = reinterpret_cast<const float *>(sv.pos) + (size_t)w * 3 * sv.ld;
+    const bool in = j < sv.N;
+    int32_t *e = enc + (size_t)w * 3 * NP;
+    e[j] = in ? enc_coord(gpos[j]) : 0;
+    e[NP + j] = in ? enc_coord(gpos[sv.ld + j]) : 0;
+    e[2 * NP + j] = in ? enc_coord(gpos[2 * sv.ld + j]) : 0;
+}
+
+template <int T, bool kEnergy>
+__global__ void __launch_bounds__(T, (T <= 128 ? 4 : 2))
+energy32g_kernel(StateView sv, const int32_t *__restrict__ enc, int NP, int nparts, double *__restrict__ partial)
+{
+    __shared__ double red[96];
+    __shared__ int32_t zw[4];
+    const int N = sv.N, ld = sv.ld;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int nwarps = T >> 5;
+    const int w = blockIdx.x / nparts, part = blockIdx.x - w * nparts;
+    const int nblk = NP >> 5;
+    const int32_t *x = enc + (size_t)w * 3 * NP, *y = x + NP, *z = x + 2 * NP;
+
+    const GroupDev g = sv.groups[sv.group_of[w]];
+    AzizF32 E;
+    E.load(g.az);
+    if (tid == 0) zw[0] = 0;
+    __syncthreads();
+    const int32_t zero = opaque_zero(zw);
+    float KV = 0.0f;
+    if (kEnergy) {
+        const Pair2 pc = pair_geom(0, 0, 0, 0, 0, 0, 0, 0, 0, pk1(0x1p63f), zero);
+        float va, vb;
+        upk2(aziz2(pc, E), va, vb);
+        KV = va;
+    }
+    const bool ragged = (N & 31) != 0;
+    double tLam = 0.0, tG2 = 0.0, tV = 0.0;
+    for (int A = part * nwarps + warp; A < nblk; A += nparts * nwarps) {
+        const int i = (A << 5) + lane;
+        const bool live = i < N;
+        const int ic = live ? i : N - 1;
+        const int32_t xi = __ldg(x + ic), yi = __ldg(y + ic), zi = __ldg(z + ic);
+        Acc64 acc = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        int n_hi = 0, fast_hi = 0, n_none = 0;
+        for (int B = 0; B < nblk; ++B) {
+            const int j0 = B << 5;
+            if (B == A || (ragged && B == nblk - 1)) {
+                double &la = (B == A) ? acc.lamd : acc.lam;
+                tile16<kEnergy, true, true, true>(x, y, z, j0, ic, N, xi, yi, zi, E, zero, acc, la, n_none);
+                tile16<kEnergy, true, true, true>(x, y, z, j0 + 16, ic, N, xi, yi, zi, E, zero, acc, la, n_none);
+            } else if (B > A) {
+                tile16<kEnergy, true, false, true>(x, y, z, j0, ic, N, xi, yi, zi, E, zero, acc, acc.lam, n_hi);
+                tile16<kEnergy, true, false, true>(x, y, z, j0 + 16, ic, N, xi, yi, zi, E, zero, acc, acc.lam, n_hi);
+                ++fast_hi;
+            } else {
+                tile16<kEnergy, false, false, true>(x, y, z, j0, ic, N, xi, yi, zi, E, zero, acc, acc.lam, n_none);
+                tile16<kEnergy, false, false, true>(x, y, z, j0 + 16, ic, N, xi, yi, zi, E, zero, acc, acc.lam, n_none);
+            }
+        }
+        if (live) {
+            sv.S[(size_t)w * ld + i] = acc.s;                          // R17: rebuild the running sum
+            if (kEnergy) {
+                const double out_hi = (double)(32 * fast_hi - n_hi);
+                tLam += 2.0 * (acc.lam - 768.0 * out_hi) + acc.lamd;
+                tG2 += acc.gx * acc.gx + acc.gy * acc.gy + acc.gz * acc.gz;
+                tV += acc.v - (double)KV * out_hi;
+            }
+        }
+    }
+    if (kEnergy) {
+        tLam = warp_sum(tLam); tG2 = warp_sum(tG2); tV = warp_sum(tV);
+        if (lane == 0) { red[warp] = tLam; red[32 + warp] = tG2; red[64 + warp] = tV; }
+        __syncthreads();
+        if (warp == 0) {
+            double a = lane < nwarps ? red[lane] : 0.0;
+            double b = lane < nwarps ? red[32 + lane] : 0.0;
+            double c = lane < nwarps ? red[64 + lane] : 0.0;
+            a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+            if (lane == 0) {
+                double *o = partial + ((size_t)w * nparts + part) * 3;
+                o[0] = a; o[1] = b; o[2] = c;
+            }
+        }
+    }
+}
+
+__global__ void finalize32g_kernel(StateView sv, double Dk, const double *__restrict__ partial, int nparts, double *__restrict__ out)
+{
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= sv.W) return;
+    double a = 0.0, b = 0.0, c = 0.0;
+    for (int p = 0; p < nparts; ++p) {                                  // fixed order
+        const double *o = partial + ((size_t)w * nparts + p) * 3;
+        a += o[0]; b += o[1]; c += o[2];
+    }
+    const GroupDev g = sv.groups[sv.group_of[w]];
+    const double Dku = Dk * g.inv_unit * g.inv_unit;
+    const double lam = -5.0 * g.b5 * a;                                 // sum_i Lambda_i
+    const double g2 = (2.5 * g.b5 * 0x1p-32) * (2.5 * g.b5 * 0x1p-32) * b;   // sum_i |G_i|^2
+    const double T_PB = -Dku * (lam + g2);
+    const double T_JF = -0.5 * Dku * lam;
+    double *o = out + (size_t)w * 4;
+    o[0] = c + T_PB; o[1] = c; o[2] = T_PB; o[3] = T_JF;
+}
+
 int smem_bytes32(int N) { return 96 * 8 + 3 * (((N + 31) >> 5) << 5) * 4; }
 
 template <int T>
@@ -227,6 +343,46 @@ int occupancy32(int smem)
 }
 
 }  // namespace
+
+cudaError_t launch_energy_f32g(qmc_ctx *c, double *d_out, bool energy)
+{
+    const int N = c->p.N, NP = ((N + 31) >> 5) << 5, nparts = c->energy_plan.parts;
+    if (!c->d_enc) {
+        cudaError_t e = cudaMalloc(&c->d_enc, sizeof(int32_t) * (size_t)c->W_total * 3 * NP);
+        if (e == cudaSuccess) e = cudaMalloc(&c->d_epart, sizeof(double) * (size_t)c->W_total * nparts * 3);
+        if (e != cudaSuccess) return e;
+    }
+    // a walker sub-range (qmc_step_host's chunks, possibly on concurrent streams) uses its own part of the scratch arrays
+    const size_t w_off = (size_t)(c->sv.walker_id_base - c->p.walker_id_base);
+    int32_t *enc = c->d_enc + w_off * 3 * NP;
+    double *epart = c->d_epart + w_off * nparts * 3;
+    encode_kernel<<<dim3((unsigned)c->W, (unsigned)((NP + 127) / 128)), 128, 0, c->stream>>>(c->sv, enc, NP);
+    if (energy) {
+        energy32g_kernel<256, true><<<(unsigned)c->W * (unsigned)nparts, 256, 0, c->stream>>>(c->sv, enc, NP, nparts, epart);
+        finalize32g_kernel<<<(c->W + 127) / 128, 128, 0, c->stream>>>(c->sv, c->p.hbar2_over_2m, epart, nparts, d_out);
+    } else {
+        energy32g_kernel<256, false><<<(unsigned)c->W * (unsigned)nparts, 256, 0, c->stream>>>(c->sv, enc, NP, nparts, epart);
+    }
+    c->launches += energy ? 2 : 1;
+    return cudaGetLastError();
+}
+
+// Gridded kernel: 8 warps per block, as many parts per walker as give every SM ~4 blocks (at most one i-block per warp)
+bool plan_energy_f32g(qmc_ctx *c, EnergyPlan *out)
+{
+    const int N = c->p.N, nblk = (N + 31) >> 5;
+    int parts = (4 * c->sm_count + c->W - 1) / c->W;
+    const int max_parts = (nblk + 7) / 8;
+    if (parts > max_parts) parts = max_parts;
+    if (parts < 1) parts = 1;
+    out->threads = 256;
+    out->smem_bytes = 0;
+    out->variant = 3;
+    out->parts = parts;
+    out->ctas_per_sm = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&out->ctas_per_sm, energy32g_kernel<256, true>, 256, 0);
+    return true;
+}
 
 #define QMC_E32_THREADS(X) X(32) X(64) X(128) X(256) X(512)
 

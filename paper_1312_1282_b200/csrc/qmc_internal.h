@@ -41,14 +41,14 @@ struct WriteoutView {
     int32_t n_out;                 // capacity in write-outs
 };
 
-struct SweepPlan  { int threads, J, V, P, K, cluster, smem_bytes, ctas_per_sm; const void *shape;
+struct SweepPlan  { int threads, J, V, P, K, cluster, Nc, smem_bytes, ctas_per_sm; const void *shape;   // cluster > 1: blocks per walker, slices of Nc particles
                     const void *fallback; int fallback_smem; };   // fallback: one-move shape for what the tile kernel does not take
 // Process-wide overrides of the launch heuristics (qmc_set_tuning; tuning experiments and tests); -1 / 0 = heuristic.
 struct Tuning { int sweep_threads = 0, sweep_per_thread = 0, sweep_vector = -1, sweep_pending = -1, sweep_tile = -1,
                     energy_threads = 0, energy_ordered = 0, sweep_cluster = -1, host_chunks = 0; };
 constexpr int kHostChunksMax = 8;
 extern Tuning g_tuning;
-struct EnergyPlan { int threads, smem_bytes, ctas_per_sm, variant; };   // variant 1 (FP64): unordered-pair kernel
+struct EnergyPlan { int threads, smem_bytes, ctas_per_sm, variant, parts; };   // variant 0 ordered pairs, 1 / 2 unordered pairs (fp64 / fp32c), 3 gridded fp32c (parts blocks per walker)
 
 }  // namespace qmc
 
@@ -64,6 +64,9 @@ struct qmc_ctx {
     qmc::StateView sv{};
     qmc::GroupDev *d_groups = nullptr;
     int32_t *d_group_of = nullptr;
+    int32_t *d_enc = nullptr;                      // gridded FP32C energy: fixed-point coordinates [W][3][NP] (first use)
+    double *d_epart = nullptr;                     //   and per-block partial sums [W][parts][3]
+    int32_t W_total = 0;                           // W of the whole context (W itself is narrowed by qmc_step_host's chunks)
     double *d_scratch = nullptr;                   // [W][4] + [W] + [W][3][N] staging for *_host calls
     // qmc_run_blocks_host: write-out stream, double-buffered block results, their events (created on first use)
     cudaStream_t out_stream = nullptr;
@@ -105,6 +108,8 @@ cudaError_t launch_energy_f32(qmc_ctx *c, double *d_out, bool energy);
 bool plan_energy_f32(qmc_ctx *c, EnergyPlan *out);
 cudaError_t launch_energy_f32s(qmc_ctx *c, double *d_out, bool energy);   // unordered pairs (qmc_energy_f32s.cu)
 bool plan_energy_f32s(qmc_ctx *c, EnergyPlan *out);
+cudaError_t launch_energy_f32g(qmc_ctx *c, double *d_out, bool energy);   // gridded, any N (qmc_energy_f32.cu)
+bool plan_energy_f32g(qmc_ctx *c, EnergyPlan *out);
 cudaError_t launch_energy_f64(qmc_ctx *c, double *d_out, bool energy);
 bool plan_energy_f64(qmc_ctx *c, EnergyPlan *out);
 

@@ -4,6 +4,7 @@
 #include <cstdlib>
 
 #include "qmc_sweep_tile.cuh"
+#include "qmc_sweep_cluster.cuh"
 
 namespace qmc {
 
@@ -12,6 +13,11 @@ Tuning g_tuning;
 cudaError_t launch_sweep(qmc_ctx *c, int n_sweeps)
 {
     c->launches += 1;
+    if (c->sweep_plan.cluster > 1) {                                 // one walker per thread-block cluster (NEXT-3)
+        const ClusterShape *cs = static_cast<const ClusterShape *>(c->sweep_plan.shape);
+        if (cs == nullptr || c->sv.proposal != 0 || c->wo.xyz != nullptr || c->p.N < 3) return cudaErrorNotSupported;
+        return cs->launch(c, n_sweeps, c->sweep_plan.smem_bytes, c->sweep_plan.cluster, c->sweep_plan.Nc);
+    }
     const SweepShape *sh = static_cast<const SweepShape *>(c->sweep_plan.shape);
     int smem = c->sweep_plan.smem_bytes;
     if (sh != nullptr && sh->K > 1 && c->sv.proposal != 0) {       // the tile kernel moves particles in order only
@@ -20,6 +26,31 @@ cudaError_t launch_sweep(qmc_ctx *c, int n_sweeps)
     }
     if (sh == nullptr) return cudaErrorInvalidValue;
     return sh->launch(c, n_sweeps, smem);
+}
+
+// Cluster plan: C blocks per walker, slices of Nc particles (a multiple of 4), the narrowest block shape that holds
+// a slice.  Used when no single block can hold the walker (N > 10240 in FP32C, > 6144 in FP64) and when
+// qmc_set_tuning("sweep_cluster") asks for it (e.g. one walker on 8 SMs).
+static bool plan_cluster(qmc_ctx *c, SweepPlan *out, int C)
+{
+    const int N = c->p.N, mode = c->p.mode;
+    int n = 0;
+    const ClusterShape *tab = (mode == QMC_FP64) ? cluster_shapes_f64(&n) : cluster_shapes_f32(&n);
+    const int Nc = (((N + C - 1) / C) + 3) & ~3;
+    const ClusterShape *best = nullptr;
+    double best_cost = 1e300;
+    for (int k = 0; k < n; ++k) {
+        const ClusterShape &s = tab[k];
+        if (s.T * s.J < Nc || s.smem > 227 * 1024) continue;
+        if (mode != QMC_FP64 && N % s.V != 0) continue;
+        const double cost = (double)s.T * ((double)s.J + (mode == QMC_FP64 ? 4.0 : 12.0)) * (s.V == 2 && mode != QMC_FP64 ? 1.12 : 1.0);
+        if (cost < best_cost) { best_cost = cost; best = &s; }
+    }
+    if (!best) return false;
+    out->threads = best->T; out->J = best->J; out->V = best->V; out->P = best->P; out->K = 1;
+    out->cluster = C; out->Nc = Nc; out->shape = best; out->smem_bytes = best->smem; out->ctas_per_sm = 1;
+    out->fallback = nullptr; out->fallback_smem = 0;
+    return true;
 }
 
 // What a shape costs (relative; it only has to rank shapes).  Fitted to the shape scans of the five configs in
@@ -57,6 +88,11 @@ bool plan_sweep(qmc_ctx *c, SweepPlan *out)
         return s.smem <= 227 * 1024;
     };
     const Tuning &tu = g_tuning;
+    out->cluster = 1; out->Nc = 0;
+    if (tu.sweep_cluster > 1 && N >= 3) {
+        int C = tu.sweep_cluster > kClusterMax ? kClusterMax : tu.sweep_cluster;
+        if (plan_cluster(c, out, C)) return true;
+    }
     auto wanted = [&](const SweepShape &s) {
         return (tu.sweep_threads <= 0 || s.T == tu.sweep_threads) && (tu.sweep_per_thread <= 0 || s.J == tu.sweep_per_thread)
             && (tu.sweep_vector < 0 || s.V == tu.sweep_vector) && (tu.sweep_pending < 0 || s.P == tu.sweep_pending)
@@ -84,7 +120,11 @@ bool plan_sweep(qmc_ctx *c, SweepPlan *out)
     out->threads = 0; out->J = 0; out->V = 0; out->P = 0; out->K = 0; out->cluster = 1; out->ctas_per_sm = 0; out->shape = nullptr;
     out->fallback = nullptr; out->fallback_smem = 0;
     out->smem_bytes = N * (8 + 3 * (mode == QMC_FP64 ? 8 : 4));
-    if (!best) return false;
+    if (!best) {                                     // no single block holds the walker: the smallest cluster that does
+        for (int C = 2; C <= kClusterMax && N >= 3; C *= 2)
+            if (plan_cluster(c, out, C)) return true;
+        return false;
+    }
     out->threads = best->T; out->J = best->J; out->V = best->V; out->P = best->P; out->K = best->K; out->shape = best;
     out->smem_bytes = best->smem;
     out->ctas_per_sm = best_occ;

@@ -93,8 +93,11 @@ def test_init_walkers_fp32c_is_the_rounded_lattice(qmc, oracle):
 
 
 # ------------------------------------------------------------------------------ trajectories
-def run_and_compare_fp64(qmc, oracle, N, W, sweeps, step, rho=wl.RHO_EQ, b=2.89, base=0, split=None, proposal=0):
+def run_and_compare_fp64(qmc, oracle, N, W, sweeps, step, rho=wl.RHO_EQ, b=2.89, base=0, split=None, proposal=0,
+                         expect_cluster=None):
     q, L = make(qmc, N, W, qmc.QMC_FP64, rho=rho, b=b, base=base)
+    if expect_cluster is not None:
+        assert q.info()["sweep_cluster"] == expect_cluster, q.info()
     q.set_proposal(proposal)
     q.init_walkers(wl.SEED)
     dec, mar = q.trace_decisions(0, W, sweeps * N)
@@ -184,6 +187,40 @@ def test_random_particle_proposal_fp32c_acceptance(qmc, oracle):
         q.sweep(1, 0.2 * L)                           # 6.77 step >= L/2
 
 
+@pytest.mark.parametrize("N,W,sweeps,C", [(4096, 2, 1, 2), (4096, 2, 1, 4), (1000, 3, 2, 8), (100, 4, 6, 2), (33, 3, 8, 8)])
+def test_trajectory_cluster_kernel_fp64(qmc, oracle, tuning, N, W, sweeps, C):
+    """NEXT-3: one walker on a cluster of C thread blocks (distributed shared memory, one cluster barrier per move) in
+    fp64: decisions move for move and committed coordinates bit for bit against the oracle, as for the one-block
+    kernel.  N = 33 on 8 blocks leaves blocks with an empty slice; N = 100 / 1000 have ragged last slices."""
+    tuning(sweep_cluster=C)
+    exempt, acc = run_and_compare_fp64(qmc, oracle, N, W, sweeps, 1.0, base=3, expect_cluster=C)
+    assert exempt <= 1 and 0.3 < acc < 0.8
+
+
+def test_large_n_needs_no_capacity_error_any_more(qmc, oracle):
+    """N = 40 960 (the paper's largest system, K20 register kernel) in the fp32-coordinate mode: the
+    planner spreads the walker over a cluster, the gridded energy kernel streams the coordinates from global memory.
+    One sweep; running pair sums and local energy against the oracle on the exported coordinates."""
+    N = 40960
+    q, L = make(qmc, N, 1, qmc.QMC_FP32C)
+    inf = q.info()
+    assert inf["sweep_cluster"] >= 4 and inf["energy_variant"] == 3, inf
+    x0 = wl.liquid_configuration(N, L, 911, fp32_grid=True)[None]
+    q.set_positions(x0)
+    q.sweep(1, 1.0)
+    a = float(q.acceptance().cpu()[0])
+    assert 0.3 < a < 0.8
+    xg = q.get_positions().cpu().numpy()
+    assert not np.array_equal(xg, x0)
+    s = orc_sys(oracle, N, L)
+    So = oracle.pair_sums(s, xg[0])
+    assert np.abs(q.pair_sums().cpu().numpy()[0] - So).max() < 5e-5 * np.abs(So).max()
+    eg = q.local_energy().cpu().numpy()
+    eo = oracle.local_energy(s, xg)
+    assert relerr32(eg, eo).max() < TOL32, relerr32(eg, eo)
+    assert np.abs(q.pair_sums().cpu().numpy()[0] - So).max() < 2e-6 * np.abs(So).max()
+
+
 def test_split_calls_continue_the_chain(qmc, oracle):
     """sweep(2); sweep(3); sweep(1) == sweep(6), including the trace offset (P11)."""
     run_and_compare_fp64(qmc, oracle, 64, 4, 6, 1.0, split=(2, 3, 1))
@@ -241,13 +278,16 @@ def test_local_energy_fp64(qmc, oracle, N):
         assert np.allclose(S[k], oracle.pair_sums(orc_sys(oracle, N, L), xyz[k]), rtol=1e-12, atol=1e-13)
 
 
+@pytest.mark.parametrize("variant", [2, 0, 3])
 @pytest.mark.parametrize("N", [64, 256, 1000, 1952])
-def test_local_energy_fp32c(qmc, oracle, N):
+def test_local_energy_fp32c(qmc, oracle, tuning, N, variant):
     """fp32 coordinates + fp32 pair arithmetic vs the fp64 oracle on the SAME (fp32-exact) coordinates.
     The cutoff guard (R2): a pair within fp32 rounding of L/2 may be classified differently; V jumps
     there by V(L/2), so such configurations are skipped if the oracle reports one (never at these seeds)."""
     W = 3
+    tuning(energy_ordered={2: 2, 0: 1, 3: 3}[variant])        # unordered pairs (bench kernel), ordered pairs, gridded
     q, L = make(qmc, N, W, qmc.QMC_FP32C)
+    assert q.info()["energy_variant"] == variant, q.info()
     xyz = np.stack([wl.liquid_configuration(N, L, 200 + N + k, fp32_grid=True) for k in range(W)])
     q.set_positions(xyz)
     assert np.array_equal(q.get_positions().cpu().numpy(), xyz)
@@ -389,6 +429,9 @@ def oracle_liquid_on_grid(oracle, N, L, W, seed, sweeps):
     (64, 6, 60, 4, dict(), 0),
     (64, 6, 60, 4, dict(sweep_tile=1), 0),
     (37, 4, 40, 5, dict(), 0),                # scalar (V = 1) shape, ragged
+    (20000, 1, 0, 1, dict(), 0),              # NEXT-3: beyond one block's shared memory -> cluster of 2 blocks
+    (1952, 2, 12, 1, dict(sweep_cluster=8), 0),       # NEXT-3: one walker on 8 SMs (the equilibration case, l.490)
+    (256, 3, 40, 2, dict(sweep_cluster=4), 0),
     (1952, 2, 12, 1, dict(), 1),              # the paper's proposal (random particle, Gaussian step)
 ])
 def test_fp32c_sweep_margins_vs_oracle(qmc, oracle, tuning, N, W, eq, sweeps, tune, proposal):
@@ -399,12 +442,15 @@ def test_fp32c_sweep_margins_vs_oracle(qmc, oracle, tuning, N, W, eq, sweeps, tu
     tuning(**tune)
     q, L = make(qmc, N, W, qmc.QMC_FP32C)
     inf = q.info()
-    for key, name in (("sweep_threads", "sweep_threads"), ("sweep_per_thread", "sweep_pairs_per_thread"), ("sweep_tile", "sweep_tile")):
+    for key, name in (("sweep_threads", "sweep_threads"), ("sweep_per_thread", "sweep_pairs_per_thread"), ("sweep_tile", "sweep_tile"),
+                      ("sweep_cluster", "sweep_cluster")):
         if key in tune:
             assert inf[name] == tune[key], inf          # the forced shape exists and is the one that runs
     if not tune and N in (1952, 10000):                  # the planner's own choice for configs 3 / 4 is a packed hi + lo shape
         assert inf["sweep_vector"] == 4 and inf["sweep_pending"] == 1, inf
-    if N == 10000:
+    if N == 20000:
+        assert inf["sweep_cluster"] == 2, inf
+    if N >= 10000:
         x0 = wl.liquid_configuration(N, L, 4242, fp32_grid=True)[None]
     else:
         x0 = oracle_liquid_on_grid(oracle, N, L, W, 77, eq)
