@@ -508,8 +508,43 @@ def main():
 
 
 def large_n_block(dev, flush):
-    """NEXT-3 figures: placeholder until the cluster kernel reports (filled in by the cluster build)."""
-    return None
+    """NEXT-3 figures (418 ms per sweep and chain at N = 40960 on a K20 -- context, not a
+    target): ms per sweep per chain at N = 40960 with the paper's 13 walkers on clusters of 8 blocks, and the single-walker case
+    (l.490) at N = 10000 and N = 1952 on a cluster of 8 against one block."""
+    import torch
+    from paper_1312_1282_b200 import binding
+
+    def timed(N, W, cluster, sweeps):
+        binding.set_tuning()
+        if cluster is not None:
+            binding.set_tuning("sweep_cluster", cluster)
+        L = wl.box_edge(N, wl.RHO_EQ)
+        q = binding.QMC(N, [W], [L], [2.89], wl.HBAR2_OVER_2M, wl.AZIZ_HFDB_HE, wl.MODE_FP32C, jitter=wl.JITTER, device=str(dev))
+        binding.set_tuning()
+        inf = q.info()
+        q.init_walkers(wl.SEED)
+        q.sweep(2, 1.0)
+        e_out = q.local_energy()
+        torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        flush.zero_()
+        ev[0].record()
+        q.sweep(sweeps, 1.0)
+        ev[1].record()
+        q.local_energy(e_out)
+        ev[2].record()
+        torch.cuda.synchronize()
+        r = {"N": N, "walkers": W, "blocks_per_walker": inf["sweep_cluster"], "threads": inf["sweep_threads"],
+             "ms_per_sweep_per_chain": ev[0].elapsed_time(ev[1]) / sweeps, "energy_ms": ev[1].elapsed_time(ev[2]),
+             "energy_variant": inf["energy_variant"], "acceptance": float(q.acceptance().mean()),
+             "pair_evals_per_s": W * N * (N - 1) * sweeps / (ev[0].elapsed_time(ev[1]) * 1e-3)}
+        q.close()
+        return r
+
+    out = {"n40960_13_walkers": timed(40960, 13, None, 1), "paper_k20_ms_per_sweep_per_chain_n40960_13_walkers": 418.0}
+    out["single_walker"] = {f"N{N}_{'cluster8' if c == 8 else 'one_block'}": timed(N, 1, c, 4 if N < 5000 else 1)
+                            for N in (10000, 1952) for c in (8, 1)}
+    return out
 
 
 if __name__ == "__main__":

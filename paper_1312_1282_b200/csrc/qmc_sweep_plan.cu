@@ -43,6 +43,7 @@ static bool plan_cluster(qmc_ctx *c, SweepPlan *out, int C)
         const ClusterShape &s = tab[k];
         if (s.T * s.J < Nc || s.smem > 227 * 1024) continue;
         if (mode != QMC_FP64 && N % s.V != 0) continue;
+        if ((g_tuning.sweep_threads > 0 && s.T != g_tuning.sweep_threads) || (g_tuning.sweep_per_thread > 0 && s.J != g_tuning.sweep_per_thread)) continue;
         const double cost = (double)s.T * ((double)s.J + (mode == QMC_FP64 ? 4.0 : 12.0)) * (s.V == 2 && mode != QMC_FP64 ? 1.12 : 1.0);
         if (cost < best_cost) { best_cost = cost; best = &s; }
     }
@@ -120,10 +121,18 @@ bool plan_sweep(qmc_ctx *c, SweepPlan *out)
     out->threads = 0; out->J = 0; out->V = 0; out->P = 0; out->K = 0; out->cluster = 1; out->ctas_per_sm = 0; out->shape = nullptr;
     out->fallback = nullptr; out->fallback_smem = 0;
     out->smem_bytes = N * (8 + 3 * (mode == QMC_FP64 ? 8 : 4));
-    if (!best) {                                     // no single block holds the walker: the smallest cluster that does
-        for (int C = 2; C <= kClusterMax && N >= 3; C *= 2)
-            if (plan_cluster(c, out, C)) return true;
-        return false;
+    // Clusters.  Few walkers of many atoms (the equilibration case): one block per walker
+    // would leave most SMs idle, and the cluster kernel's barrier pays off from N ~ 4000 (FP32C) / 2500 (FP64) up
+    // (profiles/r02_cluster.md: N = 10000, one walker: 23.0 ms per sweep on one SM, 14.4 ms on 8).  A GPC runs at
+    // most two clusters of 8, four of 4: 16 / 32 / 64 walkers at once.
+    int c_few = 1;
+    if (tu.sweep_cluster < 0 && !forced && N >= (mode == QMC_FP64 ? 2500 : 4000))
+        c_few = W <= 16 ? 8 : (W <= 32 ? 4 : (W <= 64 ? 2 : 1));
+    if (!best || c_few > 1) {                        // ... or no single block holds the walker: the smallest cluster that does
+        for (int C = (best ? c_few : 2); C <= kClusterMax && N >= 3; C *= 2)
+            if (C >= c_few && plan_cluster(c, out, C)) return true;
+        if (!best) return false;
+        out->cluster = 1; out->Nc = 0;
     }
     out->threads = best->T; out->J = best->J; out->V = best->V; out->P = best->P; out->K = best->K; out->shape = best;
     out->smem_bytes = best->smem;

@@ -420,8 +420,8 @@ def oracle_liquid_on_grid(oracle, N, L, W, seed, sweeps):
     (1952, 2, 12, 2, dict(sweep_threads=128, sweep_per_thread=16, sweep_tile=2), 0),      # tiles of 2 moves
     (1952, 2, 12, 2, dict(sweep_threads=128, sweep_per_thread=16, sweep_tile=4), 0),      # tiles of 4 moves
     (1952, 2, 12, 1, dict(sweep_threads=256, sweep_per_thread=8, sweep_tile=4), 0),
-    (10000, 1, 0, 1, dict(), 0),              # config 4: one CTA per SM, 202 KB of shared memory
-    (10000, 1, 0, 1, dict(sweep_threads=512, sweep_per_thread=20, sweep_tile=1), 0),
+    (10000, 1, 0, 1, dict(), 0),              # one walker of 10000 atoms: the planner spreads it over a cluster of 8
+    (10000, 1, 0, 1, dict(sweep_threads=512, sweep_per_thread=20, sweep_tile=1), 0),      # config 4's bench shape: one CTA per SM, 202 KB
     (10000, 1, 0, 1, dict(sweep_threads=1024, sweep_per_thread=10, sweep_tile=2), 0),     # V = 2 packs
     (256, 4, 40, 3, dict(), 0),
     (256, 4, 40, 3, dict(sweep_threads=32, sweep_per_thread=8, sweep_tile=4), 0),         # one warp: no block barrier
@@ -429,7 +429,8 @@ def oracle_liquid_on_grid(oracle, N, L, W, seed, sweeps):
     (64, 6, 60, 4, dict(), 0),
     (64, 6, 60, 4, dict(sweep_tile=1), 0),
     (37, 4, 40, 5, dict(), 0),                # scalar (V = 1) shape, ragged
-    (20000, 1, 0, 1, dict(), 0),              # NEXT-3: beyond one block's shared memory -> cluster of 2 blocks
+    (20000, 1, 0, 1, dict(), 0),              # NEXT-3: beyond one block's shared memory -> cluster (8 blocks for one walker)
+    (20000, 1, 0, 1, dict(sweep_cluster=2), 0),       #         the smallest cluster that holds it: 10000 atoms per block
     (1952, 2, 12, 1, dict(sweep_cluster=8), 0),       # NEXT-3: one walker on 8 SMs (the equilibration case, l.490)
     (256, 3, 40, 2, dict(sweep_cluster=4), 0),
     (1952, 2, 12, 1, dict(), 1),              # the paper's proposal (random particle, Gaussian step)
@@ -446,10 +447,14 @@ def test_fp32c_sweep_margins_vs_oracle(qmc, oracle, tuning, N, W, eq, sweeps, tu
                       ("sweep_cluster", "sweep_cluster")):
         if key in tune:
             assert inf[name] == tune[key], inf          # the forced shape exists and is the one that runs
-    if not tune and N in (1952, 10000):                  # the planner's own choice for configs 3 / 4 is a packed hi + lo shape
+    if not tune and N in (1952, 10000):                  # the planner's own choice is a packed hi + lo shape
         assert inf["sweep_vector"] == 4 and inf["sweep_pending"] == 1, inf
+    if not tune and N == 10000:
+        assert inf["sweep_cluster"] == 8, inf
+    if "sweep_threads" in tune:
+        assert inf["sweep_cluster"] == tune.get("sweep_cluster", 1), inf
     if N == 20000:
-        assert inf["sweep_cluster"] == 2, inf
+        assert inf["sweep_cluster"] >= 2, inf              # 20000 atoms do not fit one block's shared memory
     if N >= 10000:
         x0 = wl.liquid_configuration(N, L, 4242, fp32_grid=True)[None]
     else:
