@@ -268,6 +268,9 @@ def main():
                     help="after the timed steps: S more steps with the energy recorded, reblocked -> the paper's "
                          "t*sigma^2 and seconds to 1 mK per atom (PAPER.md l.504-511); 0 = skip")
     ap.add_argument("--large-n", action="store_true", help="add the NEXT-3 cluster-kernel figures (N = 40960, one walker on 8 SMs)")
+    ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
+                    help="qmc_set_tuning override for the headline workload, e.g. --tune sweep_tile=4 (tuning experiments; "
+                         "the defaults are the product)")
     ap.add_argument("--plumbing-only", action="store_true", help="rank plumbing only, no GPU work (CPU test of --gpus N)")
     args = ap.parse_args()
 
@@ -307,7 +310,11 @@ def main():
     K = args.steps
     sampler = ClockSampler(local) if rank == 0 else None
     equil = EQUIL_SWEEPS[args.config] if args.equil is None else args.equil
+    for kv in args.tune:
+        key, val = kv.split("=")
+        binding.set_tuning(key, int(val))
     head = Timed(w, m, dev, rank, args.proposal, args.sigma)
+    binding.set_tuning()
     head.run(equil, args.warmup, K, flush, barrier=dist.barrier if world > 1 else None, sampler=sampler)
     clocks = sampler.stop() if sampler else None
     q, steps = head.q, head.steps
@@ -399,7 +406,8 @@ def main():
                    "l2": "flushed between timed steps (256 MiB write, untimed)",
                    "equilibration_sweeps_untimed": equil,
                    "sweep_threads": info["sweep_threads"], "sweep_ctas_per_sm": info["sweep_ctas_per_sm"],
-                   "sweep_tile": info["sweep_tile"],
+                   "sweep_tile": info["sweep_tile"], "sweep_cluster": info["sweep_cluster"],
+                   "sweep_pairs_per_thread": info["sweep_pairs_per_thread"], "tuning_overrides": args.tune,
                    "energy_threads": info["energy_threads"], "energy_ctas_per_sm": info["energy_ctas_per_sm"]},
         "walker_sweeps_per_s": world * K * W * m / t_total,
         "sweep_only": {"pair_evals_per_s": world * K * sweep_pairs / t_sweep,
