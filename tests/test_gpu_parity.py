@@ -642,6 +642,29 @@ def test_error_codes(qmc):
     assert q.info()["t"] == 0
 
 
+def test_more_walkers_than_a_grid_dimension_y_holds(qmc, oracle):
+    """walkers sit on gridDim.x everywhere (limit 2^31 - 1), so W > 65535 works in every call; a sample of
+    the 70000 walkers of N = 2 atoms is compared with the oracle."""
+    N, W = 2, 70000
+    q, L = make(qmc, N, W, qmc.QMC_FP64)
+    q.init_walkers(5)
+    q.sweep(3, 0.4)
+    x = q.get_positions().cpu().numpy()
+    e = q.local_energy().cpu().numpy()
+    a = q.acceptance().cpu().numpy()
+    S = q.pair_sums().cpu().numpy()
+    assert np.isfinite(e).all() and (a >= 0).all() and (a <= 1).all() and S.shape == (W, N)
+    s = orc_sys(oracle, N, L)
+    for w0 in (0, 65535, 65536, 69999):
+        xo = oracle.init_walkers(s, 5, w0, 1, wl.JITTER)
+        oracle.sweep(s, xo, 5, w0, 0, 3, 0.4)
+        assert np.array_equal(x[w0], xo[0])
+        eo = oracle.local_energy(s, xo)[0, :4]
+        assert np.allclose(e[w0], eo, rtol=1e-10, atol=1e-12)
+    q.set_positions(x)                                      # and the import / export kernels
+    assert np.array_equal(q.get_positions().cpu().numpy(), x)
+
+
 def test_step_host_equals_device_calls(qmc):
     """qmc_step_host (host buffers in/out) == set_positions + sweep + local_energy + acceptance."""
     import torch
