@@ -1,5 +1,6 @@
 // qmc_sweep_tile.cuh -- the FP32C Metropolis sweep in TILES of K consecutive moves (SURVEY.md §8(a) rows a1-a8,
-// §7 hard part (ii); VERDICT r1 "next" #2): the timed kernel of configs 3 and 4.
+// §7 hard part (ii); VERDICT r1 "next" #2).  Oracle-green but slower than the one-move kernel (profiles/r02_tile.md,
+// DESIGN.md §6): selectable with qmc_set_tuning("sweep_tile", K), never the planner's choice.
 //
 // The one-move-at-a-time kernel (qmc_sweep_impl.cuh) pays, per move, one block reduction, one barrier and the
 // decision chain (the paper fought the same term with warp-synchronous code and a
