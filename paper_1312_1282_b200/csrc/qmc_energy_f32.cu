@@ -15,7 +15,7 @@
 // with y = 1/r, z = 1/(L-r), box units (L = 1, h = 1/2).
 //
 // No per-pair cutoff test.  r^2 is CLAMPED to h^2, where y = z = 2 exactly, so a pair at or beyond the
-// cutoff contributes exactly 0 to S_i and G_i, and exactly the constants K_L = 768 (lap term / 5 b^5) and
+// cutoff contributes exactly 0 to S_i and G_i, and exactly the constants K_L = 768 (lap term / 5 b^5; 6 in the kernel's units, qmc_energy_f32_pair.cuh) and
 // K_V = V(h) to the other two sums; the kernel counts the pairs inside the cutoff (one integer compare) and
 // removes (pairs - inside) K afterwards in fp64.  Only the j-block that contains the warp's own particles
 // (self pair, V for j > i only) and a ragged last block take a slower tile with explicit selects.
@@ -166,10 +166,10 @@ energy32_kernel(StateView sv, double Dk, double *__restrict__ out)
             }
         }
         if (live) {
-            sv.S[(size_t)w * ld + i] = acc.s;                          // R17: rebuild the running sum
+            sv.S[(size_t)w * ld + i] = acc.s * kSUnit;                 // R17: rebuild the running sum
             if (kEnergy) {
                 const double out_hi = (double)(32 * fast_hi - n_hi);
-                tLam += 2.0 * (acc.lam - 768.0 * out_hi) + acc.lamd;
+                tLam += 2.0 * (acc.lam - kLamClamp * out_hi) + acc.lamd;
                 tG2 += acc.gx * acc.gx + acc.gy * acc.gy + acc.gz * acc.gz;
                 tV += acc.v - (double)KV * out_hi;
             }
@@ -188,8 +188,8 @@ energy32_kernel(StateView sv, double Dk, double *__restrict__ out)
             if (lane == 0) {
                 // box units -> Angstrom: gradients per box edge; the minimum image carried a factor 2^32
                 const double Dku = Dk * g.inv_unit * g.inv_unit;
-                const double lam = -5.0 * g.b5 * a;                            // sum_i Lambda_i
-                const double g2 = (2.5 * g.b5 * 0x1p-32) * (2.5 * g.b5 * 0x1p-32) * b;   // sum_i |G_i|^2
+                const double lam = -5.0 * g.b5 * kGUnit * a;                            // sum_i Lambda_i
+                const double g2 = (2.5 * g.b5 * kGUnit * 0x1p-32) * (2.5 * g.b5 * kGUnit * 0x1p-32) * b;   // sum_i |G_i|^2
                 const double T_PB = -Dku * (lam + g2);
                 const double T_JF = -0.5 * Dku * lam;
                 double *o = out + (size_t)w * 4;
@@ -268,10 +268,10 @@ energy32g_kernel(StateView sv, const int32_t *__restrict__ enc, int NP, int npar
             }
         }
         if (live) {
-            sv.S[(size_t)w * ld + i] = acc.s;                          // R17: rebuild the running sum
+            sv.S[(size_t)w * ld + i] = acc.s * kSUnit;                 // R17: rebuild the running sum
             if (kEnergy) {
                 const double out_hi = (double)(32 * fast_hi - n_hi);
-                tLam += 2.0 * (acc.lam - 768.0 * out_hi) + acc.lamd;
+                tLam += 2.0 * (acc.lam - kLamClamp * out_hi) + acc.lamd;
                 tG2 += acc.gx * acc.gx + acc.gy * acc.gy + acc.gz * acc.gz;
                 tV += acc.v - (double)KV * out_hi;
             }
@@ -305,8 +305,8 @@ __global__ void finalize32g_kernel(StateView sv, double Dk, const double *__rest
     }
     const GroupDev g = sv.groups[sv.group_of[w]];
     const double Dku = Dk * g.inv_unit * g.inv_unit;
-    const double lam = -5.0 * g.b5 * a;                                 // sum_i Lambda_i
-    const double g2 = (2.5 * g.b5 * 0x1p-32) * (2.5 * g.b5 * 0x1p-32) * b;   // sum_i |G_i|^2
+    const double lam = -5.0 * g.b5 * kGUnit * a;                                 // sum_i Lambda_i
+    const double g2 = (2.5 * g.b5 * kGUnit * 0x1p-32) * (2.5 * g.b5 * kGUnit * 0x1p-32) * b;   // sum_i |G_i|^2
     const double T_PB = -Dku * (lam + g2);
     const double T_JF = -0.5 * Dku * lam;
     double *o = out + (size_t)w * 4;

@@ -8,16 +8,23 @@
 namespace qmc {
 namespace e32 {
 
-constexpr float kClamp = 0x1p62f;              // h^2 2^64
-constexpr int   kClampBits = 0x5E800000;       // bit pattern of 2^62
+// Units.  r^2 arrives as d^2 2^64 (integer differences); ONE integer instruction (VIADDMNMX: add to the exponent
+// field, then min) rescales it by 2^-62 and clamps it: a4 = min(4 r^2, 1).  Everything after that is in HALF units:
+// yh = rsqrt(a4) = y/2, q = a4 yh = 2r, zh = 1/(2 - q) = z/2; at the clamp yh = zh = q = 1.  The sums the kernels
+// keep are therefore scaled by exact powers of two, undone in fp64 at the end:
+//   pair-sum term  t/32   = yh^5 + zh^5 - 2                       (kSUnit)
+//   gradient       gm/128 = yh^7 - zh^6 yh                        (kGUnit)
+//   Laplacian      lt/128 = 2 yh^7 + 3 zh^7 + zh^6 yh = 6 at the clamp   (kGUnit, kLamClamp)
+constexpr int    kClampBits = 0x3F800000;      // bit pattern of 1.0f = the clamped a4; inside the cutoff iff bits(a4) < this
+constexpr double kSUnit = 32.0, kGUnit = 128.0, kLamClamp = 6.0;
 
 // HFD-B(HE) constants for packed fp32 evaluation.  Every constant that multiplies into the steep
 // repulsive exponential or the dispersion sum is folded (in fp64, on load) into ONE rounded coefficient
 // or carried as hi + lo, so that no fp32 rounding of a CONSTANT puts a systematic relative error on
-// every pair (the box-unit value of r_m is an arbitrary real number):
-//   rep  = eps A 2^(a1 r + a2 r^2),  a1 = -alpha log2(e) / r_m,  a2 = beta log2(e) / r_m^2   (hi + lo)
-//   disp = v^3 (k6 + v (k8 + v k10)),  v = y^2,  k_n = eps c_n r_m^n
-//   F    = 2^(-(sqrt(log2 e) max(D r_m y - 1, 0))^2)                              (D r_m hi + lo)
+// every pair (the box-unit value of r_m is an arbitrary real number).  With R = 2r and Y = y/2 (half units):
+//   rep  = eps A 2^(a1 R + a2 R^2),  a1 = -alpha log2(e) / (2 r_m),  a2 = beta log2(e) / (4 r_m^2)   (hi + lo)
+//   disp = v^3 (k6 + v (k8 + v k10)),  v = Y^2,  k_n = eps c_n r_m^n 2^n
+//   F    = 2^(-(sqrt(log2 e) max(2 D r_m Y - 1, 0))^2)                              (2 D r_m hi + lo)
 struct AzizF32 {
     f32x2 a1h, a1l, a2h, a2l, epsA, epsAln2, nk6, nk8, nk10, Dh, Dl, nDc;
     __device__ __forceinline__ void load(const AzizDev &a)
@@ -28,28 +35,33 @@ struct AzizF32 {
             hi = pk1(h);
             lo = pk1(__double2float_rn(v - (double)h));
         };
-        split(-a.alpha * a.inv_rm * log2e, a1h, a1l);
-        split(a.beta * a.inv_rm * a.inv_rm * log2e, a2h, a2l);
+        split(-0.5 * a.alpha * a.inv_rm * log2e, a1h, a1l);
+        split(0.25 * a.beta * a.inv_rm * a.inv_rm * log2e, a2h, a2l);
         const float eA = (float)(a.eps * a.A);
         epsA = pk1(eA);
         epsAln2 = pk1((float)((double)eA * ln2));
         const double r2 = a.rm2, r6 = r2 * r2 * r2;
-        nk6 = pk1((float)(-a.eps * a.c6 * r6));
-        nk8 = pk1((float)(-a.eps * a.c8 * r6 * r2));
-        nk10 = pk1((float)(-a.eps * a.c10 * r6 * r2 * r2));
-        split(a.Drm * sl, Dh, Dl);
+        nk6 = pk1((float)(-a.eps * a.c6 * r6 * 64.0));
+        nk8 = pk1((float)(-a.eps * a.c8 * r6 * r2 * 256.0));
+        nk10 = pk1((float)(-a.eps * a.c10 * r6 * r2 * r2 * 1024.0));
+        split(2.0 * a.Drm * sl, Dh, Dl);
         nDc = pk1((float)(-sl));
     }
 };
 
-// Everything the pair arithmetic of two j produces.
+// Everything the pair arithmetic of two j produces (half units, see above).
 struct Pair2 {
     f32x2 mx, my, mz;      // signed minimum image, 2^32 box units
-    f32x2 yp, q;           // y 2^-32 (hardware rsqrt), r 2^32
-    f32x2 y, z;            // 1/r, 1/(1-r)
+    f32x2 q;               // 2r
+    f32x2 y, z;            // y/2 = 1/(2r), z/2 = 1/(2(1-r))
     f32x2 y2, z2, y4, z4;
-    float a, b;            // the two lanes of min(r^2, h^2) 2^64
+    float a, b;            // the two lanes of a4 = min(4 r^2, 1)
 };
+
+__device__ __forceinline__ float scale_clamp_r2(float a)
+{
+    return __int_as_float(__viaddmin_s32(__float_as_int(a), -(62 << 23), kClampBits));
+}
 
 __device__ __forceinline__ Pair2 pair_geom(int32_t xi, int32_t yi, int32_t zi, int32_t X0, int32_t X1, int32_t Y0, int32_t Y1,
                                            int32_t Z0, int32_t Z1, f32x2 bias2, int32_t zero)
@@ -60,15 +72,14 @@ __device__ __forceinline__ Pair2 pair_geom(int32_t xi, int32_t yi, int32_t zi, i
     p.mz = pk2(__int2float_rn(wsub3(zi, Z0, zero)), __int2float_rn(wsub3(zi, Z1, zero)));
     const f32x2 r2p = fma2(p.mx, p.mx, fma2(p.my, p.my, fma2(p.mz, p.mz, bias2)));
     upk2(r2p, p.a, p.b);
-    p.a = fminf(p.a, kClamp);
-    p.b = fminf(p.b, kClamp);
-    p.yp = pk2(rsqrt_pos(p.a), rsqrt_pos(p.b));
-    p.q = mul2(pk2(p.a, p.b), p.yp);
-    const f32x2 omr = fma2(p.q, pk1(-0x1p-32f), pk1(1.0f));
-    float oa, ob;
-    upk2(omr, oa, ob);
-    p.z = pk2(rcp_pos(oa), rcp_pos(ob));
-    p.y = mul2(p.yp, pk1(0x1p32f));
+    p.a = scale_clamp_r2(p.a);
+    p.b = scale_clamp_r2(p.b);
+    p.y = pk2(rsqrt_pos(p.a), rsqrt_pos(p.b));
+    p.q = mul2(pk2(p.a, p.b), p.y);
+    const f32x2 w = fma2(p.q, pk1(-1.0f), pk1(2.0f));
+    float wa, wb;
+    upk2(w, wa, wb);
+    p.z = pk2(rcp_pos(wa), rcp_pos(wb));
     p.y2 = mul2(p.y, p.y);
     p.z2 = mul2(p.z, p.z);
     p.y4 = mul2(p.y2, p.y2);
@@ -76,17 +87,17 @@ __device__ __forceinline__ Pair2 pair_geom(int32_t xi, int32_t yi, int32_t zi, i
     return p;
 }
 
-// t = y^5 + z^5 - 64 (raw pair-sum term, u = c1 t); exactly 0 at the clamp
-__device__ __forceinline__ f32x2 pair_t(const Pair2 &p) { return fma2(p.z4, p.z, fma2(p.y4, p.y, pk1(-64.0f))); }
+// t/32 = yh^5 + zh^5 - 2 (raw pair-sum term t = y^5 + z^5 - 64, u = c1 t); exactly 0 at the clamp
+__device__ __forceinline__ f32x2 pair_t(const Pair2 &p) { return fma2(p.z4, p.z, fma2(p.y4, p.y, pk1(-2.0f))); }
 
 // HFD-B(HE) of the two pairs in K.  The hardware rsqrt is first refined by one Newton step,
-// y = y0 f with f = 3/2 - r^2 y0^2 / 2 (the seed is good to ~2^-22 and the repulsive exponential
-// amplifies a relative error of r ~11x); r = r^2 y0 f.
+// Y = yh f with f = 3/2 - q yh / 2 (the seed is good to ~2^-22 and the repulsive exponential
+// amplifies a relative error of r ~11x); R = q f = 2r.
 __device__ __forceinline__ f32x2 aziz2(const Pair2 &p, const AzizF32 &E)
 {
-    const f32x2 f = fma2(p.q, mul2(p.yp, pk1(-0.5f)), pk1(1.5f));
+    const f32x2 f = fma2(p.q, mul2(p.y, pk1(-0.5f)), pk1(1.5f));
     const f32x2 y = mul2(p.y, f);
-    const f32x2 r = mul2(mul2(p.q, pk1(0x1p-32f)), f);
+    const f32x2 r = mul2(p.q, f);
     const f32x2 v = mul2(y, y);
     const f32x2 v3 = mul2(mul2(v, v), v);
     const f32x2 ndisp = mul2(v3, fma2(v, fma2(v, E.nk10, E.nk8), E.nk6));   // -disp

@@ -7,15 +7,16 @@
 // (i_l, j_{(l+s) mod 32}) and (i_l, j_{(l+s+1) mod 32}).  G_i, S_i sums stay in the lane's registers; the terms
 // of j travel by indexed shuffles to the lanes that hold them.  Halves the special-function, integer and
 // FMA work of the ordered-pair kernel for the price of 8 shuffles per two pairs; it needs 32 more bytes of
-// shared memory per particle (fp64 per-particle accumulators), so large N keeps the ordered-pair kernel.
+// shared memory per particle (64-bit per-particle accumulators), so large N keeps the ordered-pair kernel.
 //
 // Cutoff as in qmc_energy_f32.cu: r^2 clamped to h^2, where a pair adds exactly 0 to S and G and exactly the
-// constants K_L = 768 and K_V = V(h) to the Laplacian and potential sums; clamped slots (beyond the cutoff,
-// padding particles, the inactive half of the last diagonal step: forced by a bias on r^2) are counted and
-// their constants removed in fp64.
+// constants K_L = 768 (6 in the kernel's units, qmc_energy_f32_pair.cuh) and K_V = V(h) to the Laplacian and
+// potential sums; clamped slots (beyond the cutoff, padding particles, the inactive half of the last diagonal
+// step: forced by a bias on r^2) are counted and their constants removed in fp64.
 //
 // R20: per-pair terms are fp32; at most 16 of them are summed in fp32 (two packed lanes of 8) before they are
-// added to an fp64 accumulator (per-lane accumulators for i, shared memory for j; fixed order, reproducible to the bit).
+// added to a wide accumulator: 64-bit fixed point for the per-particle sums (integer atomic adds in shared memory:
+// exact, hence independent of the order of arrival and reproducible to the bit), fp64 for the per-thread totals.
 #include "qmc_energy_f32_pair.cuh"
 
 namespace qmc {
@@ -24,14 +25,22 @@ namespace {
 
 using namespace e32;
 
-constexpr int kMaxOwn32 = 20;                        // i-blocks one warp can own (planner: ceil(nblk / nwarps) <= kMaxOwn32)
+// fixed-point grids of the per-particle accumulators: 2^-24 of a pair-sum term (t/32) and of a gradient term
+// (gm/128 times the minimum image in box units; the terms arrive times 2^32)
+constexpr double kFixS = 0x1p24, kFixG = 0x1p-8;
+__device__ __forceinline__ long long fix_s(float v) { return __float2ll_rn(v * 0x1p24f); }
+__device__ __forceinline__ long long fix_g(float v) { return __float2ll_rn(v * 0x1p-8f); }
+__device__ __forceinline__ void fix_add(long long *p, long long v)
+{
+    atomicAdd(reinterpret_cast<unsigned long long *>(p), (unsigned long long)v);
+}
 
 __device__ __forceinline__ float shfl_f(float v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 
 struct SymAcc {            // fp32 partial sums of up to 8 packed steps
     f32x2 gxi, gyi, gzi, si;       // this lane's particle i
     f32x2 gxj, gyj, gzj, sj;       // the particle j this lane holds
-    f32x2 lam, v;                  // totals
+    f32x2 lam, lg, v;              // totals: y^7 + z^7, gm, V
 };
 
 // Eight packed steps (16 pairs) of one block pair, starting at step s0 (step s pairs lane l with j-lane (l+s) & 31).
@@ -62,9 +71,11 @@ __device__ __forceinline__ void sym_steps16(const int32_t *__restrict__ x, const
         const int fa = (lane - sa) & 31, fb = (lane - sb) & 31;
         P.sj = add2(P.sj, pk2(shfl_f(t0, fa), shfl_f(t1, fb)));
         if (kEnergy) {
+            // gm = (y^6 - z^6) y;  Laplacian term 2 y^7 + 3 z^7 + z^6 y = 3 (y^7 + z^7) - gm: the two sums are kept apart
             const f32x2 y6 = mul2(q.y4, q.y2), z6 = mul2(q.z4, q.z2);
-            const f32x2 y7 = mul2(y6, q.y), z6y = mul2(z6, q.y), z7 = mul2(z6, q.z);
-            const f32x2 gm = sub2(y7, z6y);
+            const f32x2 gm = mul2(sub2(y6, z6), q.y);
+            P.lam = fma2(z6, q.z, fma2(y6, q.y, P.lam));
+            P.lg = add2(P.lg, gm);
             const f32x2 cx = mul2(gm, q.mx), cy = mul2(gm, q.my), cz = mul2(gm, q.mz);
             P.gxi = add2(P.gxi, cx);
             P.gyi = add2(P.gyi, cy);
@@ -76,14 +87,13 @@ __device__ __forceinline__ void sym_steps16(const int32_t *__restrict__ x, const
             P.gxj = add2(P.gxj, pk2(shfl_f(a0, fa), shfl_f(a1, fb)));      // subtracted when flushed (d_ji = -d_ij)
             P.gyj = add2(P.gyj, pk2(shfl_f(b0, fa), shfl_f(b1, fb)));
             P.gzj = add2(P.gzj, pk2(shfl_f(c0, fa), shfl_f(c1, fb)));
-            P.lam = add2(P.lam, fma2(y7, pk1(2.0f), fma2(z7, pk1(3.0f), z6y)));
             P.v = add2(P.v, aziz2(q, E));
         }
     }
 }
 
 template <int T, bool kEnergy>
-__global__ void __launch_bounds__(T, (T <= 128 ? 4 : (T <= 256 ? 2 : 1)))
+__global__ void __launch_bounds__(T, (T <= 128 ? 4 : (T <= 384 ? 2 : 1)))
 energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -95,7 +105,7 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
 
     double  *red = reinterpret_cast<double *>(smem_raw);              // [3][32]
                                                                       // red[97]: opaque zero
-    double  *ag  = red + 98;                                          // [4][NP]: G_x, G_y, G_z (2^32 box units), S
+    long long *ag = reinterpret_cast<long long *>(red + 98);          // [4][NP]: G_x, G_y, G_z, S as fixed point
     int32_t *x   = reinterpret_cast<int32_t *>(ag + 4 * NP);          // [3][NP]
     int32_t *y = x + NP, *z = x + 2 * NP;
 
@@ -109,7 +119,7 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
         x[j] = in ? enc_coord(gpos[j]) : 0;
         y[j] = in ? enc_coord(gpos[ld + j]) : 0;
         z[j] = in ? enc_coord(gpos[2 * ld + j]) : 0;
-        ag[j] = 0.0; ag[NP + j] = 0.0; ag[2 * NP + j] = 0.0; ag[3 * NP + j] = 0.0;
+        ag[j] = 0; ag[NP + j] = 0; ag[2 * NP + j] = 0; ag[3 * NP + j] = 0;
     }
     if (tid == 0) *reinterpret_cast<int32_t *>(red + 97) = 0;
     __syncthreads();
@@ -123,89 +133,77 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
         KV = va;
     }
 
-    // Schedule as in qmc_energy_f64.cu (deterministic): warp v owns the i-blocks A = v, v + nwarps, ...;
-    // all warps step through the ring offsets k together (one barrier per offset), so within one offset the j-blocks
-    // B = A + k of different warps are different and the j-side sums are added to shared memory by plain
-    // read-modify-writes in the order of k; the i-side sums wait in local accumulators until the last offset.
+    // Schedule (deterministic): the block pairs (A, B = A + k), k = 0 .. K (+ the offset n/2 once per pair for
+    // even n), form one flat task list that the warps take round-robin -- a fixed set in a fixed order per warp, so the
+    // per-thread totals are reproducible.  The per-particle sums of BOTH blocks of a task go to shared memory as 64-bit
+    // FIXED-POINT numbers by integer atomic adds: integer addition is associative, so the result does not depend on the
+    // order in which the warps arrive, and the main loop needs no barrier at all (round 2's per-offset barrier and
+    // thread-local accumulator arrays are gone).  The fixed-point grid is 2^-24 of the kernel's units (kFixS, kFixG):
+    // finer than the fp32 partial sums that are added to it (|partial| >= 1 converts exactly), 63 bits of range.
     const int K = (nblk - 1) >> 1;
     const bool even = (nblk & 1) == 0, ragged = (N & 31) != 0;
-    double tLam = 0.0, tV = 0.0;
+    const int nfull = nblk * (K + 1), ntask = nfull + (even ? (nblk >> 1) : 0);
+    double tLam = 0.0, tLg = 0.0, tV = 0.0;
     long long slots = 0, inside = 0;
-    double own[kMaxOwn32][4];                                         // G_x, G_y, G_z, S of this lane's particle in each own block
 #pragma unroll 1
-    for (int a = 0; a < kMaxOwn32; ++a) { own[a][0] = 0.0; own[a][1] = 0.0; own[a][2] = 0.0; own[a][3] = 0.0; }
-    const int kend = K + (even ? 1 : 0);
-#pragma unroll 1
-    for (int k = 0; k <= kend; ++k) {
-        int a = 0;
-#pragma unroll 1
-        for (int A = warp; A < nblk; A += nwarps, ++a) {
-            if (k > K && A >= (nblk >> 1)) break;                    // even n: the offset n/2 once per block pair
-            const int i = (A << 5) + lane;
-            const bool vi = i < N;
-            const int32_t xi = x[i], yi = y[i], zi = z[i];
-            double gxi = 0.0, gyi = 0.0, gzi = 0.0, si = 0.0;
-            int B = A + k;
-            if (B >= nblk) B -= nblk;
-            const int jb = B << 5;
-            const bool diag = (k == 0);
-            const bool bias = diag || (ragged && (A == nblk - 1 || B == nblk - 1));
-            double gxj = 0.0, gyj = 0.0, gzj = 0.0, sj = 0.0;
-            const int nhalf = diag ? 1 : 2;
-            for (int hlf = 0; hlf < nhalf; ++hlf) {
-                SymAcc P;
-                P.gxi = P.gyi = P.gzi = P.si = P.gxj = P.gyj = P.gzj = P.sj = P.lam = P.v = pk1(0.0f);
-                int n_in = 0;
-                const int s0 = diag ? 1 : 16 * hlf;
-                if (bias) sym_steps16<kEnergy, true>(x, y, z, jb, s0, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
-                else      sym_steps16<kEnergy, false>(x, y, z, jb, s0, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
-                slots += 16; inside += n_in;
-                si += (double)hsum2(P.si);
-                sj += (double)hsum2(P.sj);
-                if (kEnergy) {
-                    gxi += (double)hsum2(P.gxi); gyi += (double)hsum2(P.gyi); gzi += (double)hsum2(P.gzi);
-                    gxj += (double)hsum2(P.gxj); gyj += (double)hsum2(P.gyj); gzj += (double)hsum2(P.gzj);
-                    tLam += (double)hsum2(P.lam);
-                    tV += (double)hsum2(P.v);
-                }
+    for (int t = warp; t < ntask; t += nwarps) {
+        int k, A;
+        if (t < nfull) { k = t / nblk; A = t - k * nblk; }
+        else           { k = K + 1; A = t - nfull; }                 // even n: the offset n/2 once per block pair
+        const int i = (A << 5) + lane;
+        const bool vi = i < N;
+        const int32_t xi = x[i], yi = y[i], zi = z[i];
+        int B = A + k;
+        if (B >= nblk) B -= nblk;
+        const int jb = B << 5;
+        const bool diag = (k == 0);
+        const bool bias = diag || (ragged && (A == nblk - 1 || B == nblk - 1));
+        long long gxi = 0, gyi = 0, gzi = 0, si = 0, gxj = 0, gyj = 0, gzj = 0, sj = 0;
+        const int nhalf = diag ? 1 : 2;
+        for (int hlf = 0; hlf < nhalf; ++hlf) {
+            SymAcc P;
+            P.gxi = P.gyi = P.gzi = P.si = P.gxj = P.gyj = P.gzj = P.sj = P.lam = P.lg = P.v = pk1(0.0f);
+            int n_in = 0;
+            const int s0 = diag ? 1 : 16 * hlf;
+            if (bias) sym_steps16<kEnergy, true>(x, y, z, jb, s0, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
+            else      sym_steps16<kEnergy, false>(x, y, z, jb, s0, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
+            slots += 16; inside += n_in;
+            si += fix_s(hsum2(P.si));
+            sj += fix_s(hsum2(P.sj));
+            if (kEnergy) {
+                gxi += fix_g(hsum2(P.gxi)); gyi += fix_g(hsum2(P.gyi)); gzi += fix_g(hsum2(P.gzi));
+                gxj += fix_g(hsum2(P.gxj)); gyj += fix_g(hsum2(P.gyj)); gzj += fix_g(hsum2(P.gzj));
+                tLam += (double)hsum2(P.lam);
+                tLg += (double)hsum2(P.lg);
+                tV += (double)hsum2(P.v);
             }
-            if (jb + lane < N) {
-                ag[3 * NP + jb + lane] += sj;
-                if (kEnergy) {
-                    ag[jb + lane] -= gxj;
-                    ag[NP + jb + lane] -= gyj;
-                    ag[2 * NP + jb + lane] -= gzj;
-                }
-            }
-            own[a][3] += si;
-            if (kEnergy) { own[a][0] += gxi; own[a][1] += gyi; own[a][2] += gzi; }
         }
-        __syncthreads();
-    }
-    {
-        int a = 0;
-#pragma unroll 1
-        for (int A = warp; A < nblk; A += nwarps, ++a) {
-            const int i = (A << 5) + lane;
-            if (i < N) {
-                ag[3 * NP + i] += own[a][3];
-                if (kEnergy) { ag[i] += own[a][0]; ag[NP + i] += own[a][1]; ag[2 * NP + i] += own[a][2]; }
+        if (jb + lane < N) {
+            fix_add(ag + 3 * NP + jb + lane, sj);
+            if (kEnergy) {
+                fix_add(ag + jb + lane, -gxj);                        // d_ji = -d_ij
+                fix_add(ag + NP + jb + lane, -gyj);
+                fix_add(ag + 2 * NP + jb + lane, -gzj);
             }
+        }
+        if (vi) {
+            fix_add(ag + 3 * NP + i, si);
+            if (kEnergy) { fix_add(ag + i, gxi); fix_add(ag + NP + i, gyi); fix_add(ag + 2 * NP + i, gzi); }
         }
     }
     __syncthreads();
 
     double tG2 = 0.0;
     for (int i = tid; i < N; i += T) {
-        sv.S[(size_t)w * ld + i] = ag[3 * NP + i];                    // R17: rebuild the running sum
+        sv.S[(size_t)w * ld + i] = (double)ag[3 * NP + i] * (kSUnit / kFixS);      // R17: rebuild the running sum
         if (kEnergy) {
-            const double a = ag[i], b = ag[NP + i], c = ag[2 * NP + i];
+            const double a = (double)ag[i] * (1.0 / kFixG), b = (double)ag[NP + i] * (1.0 / kFixG), c = (double)ag[2 * NP + i] * (1.0 / kFixG);
             tG2 += a * a + b * b + c * c;
         }
     }
     if (kEnergy) {
         const double n_out = (double)(slots - inside);
-        tLam = 2.0 * (tLam - 768.0 * n_out);                          // each unordered pair seen once
+        tLam = 2.0 * (3.0 * (tLam - 2.0 * n_out) - tLg);              // each unordered pair seen once; a clamped slot adds y^7 + z^7 = 2, gm = 0
         tV -= (double)KV * n_out;
         tLam = warp_sum(tLam); tG2 = warp_sum(tG2); tV = warp_sum(tV);
         if (lane == 0) { red[warp] = tLam; red[32 + warp] = tG2; red[64 + warp] = tV; }
@@ -217,8 +215,8 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
             a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
             if (lane == 0) {
                 const double Dku = Dk * g.inv_unit * g.inv_unit;
-                const double lam = -5.0 * g.b5 * a;                                     // sum_i Lambda_i
-                const double g2 = (2.5 * g.b5 * 0x1p-32) * (2.5 * g.b5 * 0x1p-32) * b;   // sum_i |G_i|^2
+                const double lam = -5.0 * g.b5 * kGUnit * a;                            // sum_i Lambda_i
+                const double g2 = (2.5 * g.b5 * kGUnit * 0x1p-32) * (2.5 * g.b5 * kGUnit * 0x1p-32) * b;   // sum_i |G_i|^2
                 const double T_PB = -Dku * (lam + g2);
                 const double T_JF = -0.5 * Dku * lam;
                 double *o = out + (size_t)w * 4;
@@ -259,7 +257,7 @@ int occupancy32s(int smem)
 
 }  // namespace
 
-#define QMC_E32S_THREADS(X) X(32) X(64) X(128) X(256) X(512)
+#define QMC_E32S_THREADS(X) X(32) X(64) X(128) X(256) X(384) X(512)
 
 cudaError_t launch_energy_f32s(qmc_ctx *c, double *d_out, bool energy)
 {
@@ -281,11 +279,8 @@ bool plan_energy_f32s(qmc_ctx *c, EnergyPlan *out)
     while (2 * T < N && T < 256) T *= 2;
     if (g_tuning.energy_threads > 0) {
         const int v = g_tuning.energy_threads;
-        if (v >= 32 && v <= 512 && (v & (v - 1)) == 0) T = v;
+        if (v >= 32 && v <= 512 && ((v & (v - 1)) == 0 || v == 384)) T = v;
     }
-    const int nblk = (N + 31) >> 5;
-    while ((nblk + (T >> 5) - 1) / (T >> 5) > kMaxOwn32 && T < 512) T *= 2;     // own-block accumulators per warp
-    if ((nblk + (T >> 5) - 1) / (T >> 5) > kMaxOwn32) return false;
     out->threads = T;
     out->smem_bytes = smem;
     out->variant = 2;

@@ -78,7 +78,8 @@ sweep_cluster_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_s
     const GroupDev g = sv.groups[sv.group_of[w]];
     SweepConst<Real> P;
     P.load(g);
-    const double c2 = 2.0 * g.c1;
+    constexpr double kUnit = kPacked ? kT2Unit : 1.0, kInvUnit = 1.0 / kUnit;   // packed FP32C sums are in units of kT2Unit
+    const double c2 = 2.0 * g.c1 * kUnit;
     const double step = kF32 ? g.step * g.inv_unit * 8388608.0 : g.step;
     const uint32_t wid = sv.walker_id_base + (uint32_t)w;
 
@@ -92,7 +93,7 @@ sweep_cluster_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_s
             const int j = j0 + l;
             if constexpr (kF32) { cx = enc_coord(gpos[j]); cy = enc_coord(gpos[ld + j]); cz = enc_coord(gpos[2 * ld + j]); }
             else                { cx = gpos[j]; cy = gpos[ld + j]; cz = gpos[2 * ld + j]; }
-            s = gS[j];
+            s = gS[j] * kInvUnit;
         } else {
             if constexpr (kF32) { cx = 0; cy = 0; cz = 0; }
             else                { cx = cy = cz = poison_of<Real>(Coord(0)); }
@@ -345,8 +346,8 @@ sweep_cluster_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_s
         const int j = j0 + l;
         if constexpr (kF32) { gpos[j] = dec_coord(x[l]); gpos[ld + j] = dec_coord(y[l]); gpos[2 * ld + j] = dec_coord(z[l]); }
         else                { gpos[j] = x[l]; gpos[ld + j] = y[l]; gpos[2 * ld + j] = z[l]; }
-        if constexpr (kPend) gS[j] = (double)Shi[l] + (double)Slo[l];
-        else                 gS[j] = S[s_index<T, V>(l)];
+        if constexpr (kPend) gS[j] = ((double)Shi[l] + (double)Slo[l]) * kUnit;
+        else                 gS[j] = S[s_index<T, V>(l)] * kUnit;
     }
     if (rank == 0 && tid == 0) sv.n_acc[w] += n_acc;
 }

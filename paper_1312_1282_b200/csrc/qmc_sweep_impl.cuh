@@ -93,10 +93,20 @@ __device__ __forceinline__ float pair_t(int32_t px, int32_t py, int32_t pz, int3
     return fmaf(z4, z, fmaf(y4, y, -64.0f));
 }
 
-// Two FP32C pair terms at once: same arithmetic as pair_t(int...) but r^2 stays scaled by 2^64 up to the
-// reciprocal square root (y' = y 2^-32, q = r 2^32), which saves the scaling multiply; the clamp is at
-// 2^62 = h^2 2^64 and bias2 holds 0 or 2^63 per lane (padding).  Every power of two is exact, so the
-// results are bit-identical to the scalar form.
+// Two FP32C pair terms at once, in units of 32: returns t/32 = (y/2)^5 + (z/2)^5 - 2.
+// r^2 arrives as d^2 2^64 (integer differences); ONE integer instruction (VIADDMNMX: add to the exponent
+// field, then min) rescales it by 2^-62 and clamps it: a4 = min(4 r^2, 1).  Then yh = rsqrt(a4) = y/2,
+// q = a4 yh = 2r, w = 2 - q = 2(1 - r), zh = 1/w = z/2; at the clamp yh = zh = 1 and t/32 = 0 exactly.
+// bias2 holds 0 or 2^63 per lane (padding: clamps).  Every scale factor is a power of two (and an even one
+// in front of the reciprocal square root), so 32 x the result is bit-identical to the scalar form; the
+// packed kernels keep their sums in these units (kT2Unit) and convert on load / store.
+// d != 0 means d^2 2^64 >= 1, so the exponent subtraction cannot underflow; d = 0 (two particles on one grid
+// point) gives a negative number, rsqrt = NaN, and the move is rejected as it was with y = inf.
+constexpr double kT2Unit = 32.0;
+__device__ __forceinline__ float scale_clamp_r2(float a)
+{
+    return __int_as_float(__viaddmin_s32(__float_as_int(a), -(62 << 23), 0x3F800000));
+}
 __device__ __forceinline__ f32x2 pair_t2(int32_t px, int32_t py, int32_t pz, int32_t X0, int32_t X1, int32_t Y0, int32_t Y1,
                                          int32_t Z0, int32_t Z1, f32x2 bias2, int32_t zero)
 {
@@ -106,19 +116,17 @@ __device__ __forceinline__ f32x2 pair_t2(int32_t px, int32_t py, int32_t pz, int
     const f32x2 r2p = fma2(mx, mx, fma2(my, my, fma2(mz, mz, bias2)));
     float a, b;
     upk2(r2p, a, b);
-    a = fminf(a, 0x1p62f);
-    b = fminf(b, 0x1p62f);
-    const float ya = rsqrt_pos(a), yb = rsqrt_pos(b);                   // y 2^-32
-    const f32x2 r2c = pk2(a, b), yp = pk2(ya, yb);
-    const f32x2 q = mul2(r2c, yp);                                      // r 2^32
-    const f32x2 omr = fma2(q, pk2(-0x1p-32f, -0x1p-32f), pk2(1.0f, 1.0f));
-    float oa, ob;
-    upk2(omr, oa, ob);
-    const f32x2 z = pk2(rcp_pos(oa), rcp_pos(ob));
-    const f32x2 y = mul2(yp, pk2(0x1p32f, 0x1p32f));
+    a = scale_clamp_r2(a);
+    b = scale_clamp_r2(b);
+    const f32x2 y = pk2(rsqrt_pos(a), rsqrt_pos(b));                    // y/2
+    const f32x2 q = mul2(pk2(a, b), y);                                 // 2r
+    const f32x2 w = fma2(q, pk2(-1.0f, -1.0f), pk2(2.0f, 2.0f));
+    float wa, wb;
+    upk2(w, wa, wb);
+    const f32x2 z = pk2(rcp_pos(wa), rcp_pos(wb));                      // z/2
     const f32x2 y2 = mul2(y, y), z2 = mul2(z, z);
     const f32x2 y4 = mul2(y2, y2), z4 = mul2(z2, z2);
-    return fma2(z4, z, fma2(y4, y, pk2(-64.0f, -64.0f)));
+    return fma2(z4, z, fma2(y4, y, pk2(-2.0f, -2.0f)));
 }
 
 template <typename Real> __device__ __forceinline__ typename ModeT<Real>::Coord poison_of(typename ModeT<Real>::Coord p);
@@ -256,7 +264,9 @@ sweep_kernel(StateView sv, TraceView tr, WriteoutView wo, uint2 key, uint32_t t0
     const GroupDev g = sv.groups[sv.group_of[w]];
     SweepConst<Real> P;
     P.load(g);
-    const double c2 = 2.0 * g.c1;                          // 2 Delta = c2 * (sum t_new - S_s)
+    // 2 Delta = c2 * (sum t_new - S_s); the packed FP32C path keeps every sum in units of kT2Unit
+    constexpr double kUnit = kPacked ? kT2Unit : 1.0, kInvUnit = 1.0 / kUnit;
+    const double c2 = 2.0 * g.c1 * kUnit;
     // proposal half-width: FP64 exactly the caller's step [A]; FP32C in grid units (2^-23 box)
     const double step = kF32 ? g.step * g.inv_unit * 8388608.0 : g.step;
     const uint32_t wid = sv.walker_id_base + (uint32_t)w;
@@ -270,7 +280,7 @@ sweep_kernel(StateView sv, TraceView tr, WriteoutView wo, uint2 key, uint32_t t0
         if (j < N) {
             if constexpr (kF32) { cx = enc_coord(gpos[j]); cy = enc_coord(gpos[ld + j]); cz = enc_coord(gpos[2 * ld + j]); }
             else                { cx = gpos[j]; cy = gpos[ld + j]; cz = gpos[2 * ld + j]; }
-            s = gS[j];
+            s = gS[j] * kInvUnit;
         } else {                                            // padding: NaN selects 0 in FP64; FP32C uses the bias
             if constexpr (kF32) { cx = 0; cy = 0; cz = 0; }
             else                { cx = cy = cz = poison_of<Real>(Coord(0)); }
@@ -544,8 +554,8 @@ sweep_kernel(StateView sv, TraceView tr, WriteoutView wo, uint2 key, uint32_t t0
     for (int j = tid; j < N; j += T) {
         if constexpr (kF32) { gpos[j] = dec_coord(x[j]); gpos[ld + j] = dec_coord(y[j]); gpos[2 * ld + j] = dec_coord(z[j]); }
         else                { gpos[j] = x[j]; gpos[ld + j] = y[j]; gpos[2 * ld + j] = z[j]; }
-        if constexpr (kPend) gS[j] = (double)Shi[j] + (double)Slo[j];
-        else                 gS[j] = S[s_index<T, V>(j)];
+        if constexpr (kPend) gS[j] = ((double)Shi[j] + (double)Slo[j]) * kUnit;
+        else                 gS[j] = S[s_index<T, V>(j)] * kUnit;
     }
     if (tid == 0) sv.n_acc[w] += n_acc;
 }

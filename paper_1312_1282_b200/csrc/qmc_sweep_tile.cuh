@@ -117,7 +117,7 @@ sweep_tile_kernel(StateView sv, TraceView tr, WriteoutView wo, uint2 key, uint32
     int32_t *y = x + NP, *z = x + 2 * NP;
 
     const GroupDev g = sv.groups[sv.group_of[w]];
-    const double c2 = 2.0 * g.c1;                          // 2 Delta = c2 * (sum t_new - S_s)
+    const double c2 = 2.0 * g.c1 * kT2Unit;                // 2 Delta = c2 * (sum t_new - S_s), sums in units of kT2Unit (pair_t2)
     const double step = g.step * g.inv_unit * 8388608.0;   // proposal half-width in grid units (2^-23 box)
     const uint32_t wid = sv.walker_id_base + (uint32_t)w;
 
@@ -129,7 +129,7 @@ sweep_tile_kernel(StateView sv, TraceView tr, WriteoutView wo, uint2 key, uint32
         double s = 0.0;
         if (j < N) {
             cx = enc_coord(gpos[j]); cy = enc_coord(gpos[ld + j]); cz = enc_coord(gpos[2 * ld + j]);
-            s = gS[j];
+            s = gS[j] * (1.0 / kT2Unit);
         }
         x[j] = cx; y[j] = cy; z[j] = cz;
         const float hi = __double2float_rn(s);
@@ -208,7 +208,7 @@ sweep_tile_kernel(StateView sv, TraceView tr, WriteoutView wo, uint2 key, uint32
             if (ta) { ax = wadd(ax, rdx[ra]); ay = wadd(ay, rdy[ra]); az = wadd(az, rdz[ra]); }
             if (tb) { bx = wadd(bx, rdx[rb]); by = wadd(by, rdy[rb]); bz = wadd(bz, rdz[rb]); }
             const SweepConst<float> P0{};
-            corr[buf * 32 + lane] = pair_t(ax, ay, az, bx, by, bz, 0.0f, P0);
+            corr[buf * 32 + lane] = pair_t(ax, ay, az, bx, by, bz, 0.0f, P0) * (float)(1.0 / kT2Unit);
         }
 
         int s0n = s0 + K;
@@ -390,7 +390,7 @@ sweep_tile_kernel(StateView sv, TraceView tr, WriteoutView wo, uint2 key, uint32
     // a8: shared -> global, once per call
     for (int j = tid; j < N; j += T) {
         gpos[j] = dec_coord(x[j]); gpos[ld + j] = dec_coord(y[j]); gpos[2 * ld + j] = dec_coord(z[j]);
-        gS[j] = (double)Shi[j] + (double)Slo[j];
+        gS[j] = ((double)Shi[j] + (double)Slo[j]) * kT2Unit;
     }
     if (tid == 0) sv.n_acc[w] += n_acc;
 }
