@@ -14,9 +14,10 @@
 // potential sums; clamped slots (beyond the cutoff, padding particles, the inactive half of the last diagonal
 // step: forced by a bias on r^2) are counted and their constants removed in fp64.
 //
-// R20: per-pair terms are fp32; at most 16 of them are summed in fp32 (two packed lanes of 8) before they are
-// added to a wide accumulator: 64-bit fixed point for the per-particle sums (integer atomic adds in shared memory:
-// exact, hence independent of the order of arrival and reproducible to the bit), fp64 for the per-thread totals.
+// R20: per-pair terms are fp32; a packed lane sums at most 16 of them in fp32, the two lanes are added (32 terms, one
+// block pair) and the result goes to a wide accumulator: 64-bit fixed point for the per-particle sums (integer
+// atomic adds in shared memory: exact, hence independent of the order of arrival and reproducible to the bit), fp64
+// for the per-thread totals.
 #include "qmc_energy_f32_pair.cuh"
 
 namespace qmc {
@@ -30,29 +31,39 @@ using namespace e32;
 constexpr double kFixS = 0x1p24, kFixG = 0x1p-8;
 __device__ __forceinline__ long long fix_s(float v) { return __float2ll_rn(v * 0x1p24f); }
 __device__ __forceinline__ long long fix_g(float v) { return __float2ll_rn(v * 0x1p-8f); }
-__device__ __forceinline__ void fix_add(long long *p, long long v)
+// A 64-bit fixed-point accumulator is two 32-bit words, hi (signed, units of 2^24) and lo (unsigned): v = hi 2^24 +
+// lo with 0 <= lo < 2^24 is added by TWO native 32-bit shared-memory atomics (a 64-bit atomic add on shared memory is
+// a compare-and-swap loop).  A particle receives at most nblk + 1 <= 81 additions, so lo stays below 2^31 and no
+// carry is ever lost; fix_get() puts the words together.
+__device__ __forceinline__ void fix_add(int32_t *ag, int idx, long long v)
 {
-    atomicAdd(reinterpret_cast<unsigned long long *>(p), (unsigned long long)v);
+    atomicAdd(ag + 2 * idx, (int32_t)(v >> 24));
+    atomicAdd(reinterpret_cast<uint32_t *>(ag) + 2 * idx + 1, (uint32_t)v & 0xFFFFFFu);
+}
+__device__ __forceinline__ double fix_get(const int32_t *ag, int idx)
+{
+    return (double)(((long long)ag[2 * idx] << 24) + (long long)reinterpret_cast<const uint32_t *>(ag)[2 * idx + 1]);
 }
 
 __device__ __forceinline__ float shfl_f(float v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 
-struct SymAcc {            // fp32 partial sums of up to 8 packed steps
+struct SymAcc {            // fp32 partial sums of up to 16 packed steps
     f32x2 gxi, gyi, gzi, si;       // this lane's particle i
     f32x2 gxj, gyj, gzj, sj;       // the particle j this lane holds
     f32x2 lam, lg, v;              // totals: y^7 + z^7, gm, V
 };
 
-// Eight packed steps (16 pairs) of one block pair, starting at step s0 (step s pairs lane l with j-lane (l+s) & 31).
+// npk packed steps (2 npk pairs) of one block pair, starting at step s0 (step s pairs lane l with j-lane (l+s) & 31):
+// npk = 16, s0 = 0 for a full block pair, npk = 8, s0 = 1 for the diagonal block.
 //   kBias: some slots must be forced beyond the cutoff (padding particles, second half of diagonal step 16)
 template <bool kEnergy, bool kBias>
-__device__ __forceinline__ void sym_steps16(const int32_t *__restrict__ x, const int32_t *__restrict__ y, const int32_t *__restrict__ z,
-                                            int jb, int s0, int lane, bool vi, int N, bool diag,
+__device__ __forceinline__ void sym_steps(const int32_t *__restrict__ x, const int32_t *__restrict__ y, const int32_t *__restrict__ z,
+                                            int jb, int s0, int npk, int lane, bool vi, int N, bool diag,
                                             int32_t xi, int32_t yi, int32_t zi, const AzizF32 &E, int32_t zero,
                                             SymAcc &P, int &n_in)
 {
 #pragma unroll 2
-    for (int p = 0; p < 8; ++p) {
+    for (int p = 0; p < npk; ++p) {
         const int sa = s0 + 2 * p, sb = sa + 1;
         const int ja = (lane + sa) & 31, jl = (lane + sb) & 31;
         f32x2 bias2 = pk1(0.0f);
@@ -105,8 +116,8 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
 
     double  *red = reinterpret_cast<double *>(smem_raw);              // [3][32]
                                                                       // red[97]: opaque zero
-    long long *ag = reinterpret_cast<long long *>(red + 98);          // [4][NP]: G_x, G_y, G_z, S as fixed point
-    int32_t *x   = reinterpret_cast<int32_t *>(ag + 4 * NP);          // [3][NP]
+    int32_t *ag = reinterpret_cast<int32_t *>(red + 98);              // [4][NP][2]: G_x, G_y, G_z, S as fixed point (hi, lo)
+    int32_t *x   = ag + 8 * NP;                                       // [3][NP]
     int32_t *y = x + NP, *z = x + 2 * NP;
 
     const GroupDev g = sv.groups[sv.group_of[w]];
@@ -119,7 +130,10 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
         x[j] = in ? enc_coord(gpos[j]) : 0;
         y[j] = in ? enc_coord(gpos[ld + j]) : 0;
         z[j] = in ? enc_coord(gpos[2 * ld + j]) : 0;
-        ag[j] = 0; ag[NP + j] = 0; ag[2 * NP + j] = 0; ag[3 * NP + j] = 0;
+        *reinterpret_cast<int2 *>(ag + 2 * j) = make_int2(0, 0);
+        *reinterpret_cast<int2 *>(ag + 2 * (NP + j)) = make_int2(0, 0);
+        *reinterpret_cast<int2 *>(ag + 2 * (2 * NP + j)) = make_int2(0, 0);
+        *reinterpret_cast<int2 *>(ag + 2 * (3 * NP + j)) = make_int2(0, 0);
     }
     if (tid == 0) *reinterpret_cast<int32_t *>(red + 97) = 0;
     __syncthreads();
@@ -142,14 +156,12 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
     // finer than the fp32 partial sums that are added to it (|partial| >= 1 converts exactly), 63 bits of range.
     const int K = (nblk - 1) >> 1;
     const bool even = (nblk & 1) == 0, ragged = (N & 31) != 0;
-    const int nfull = nblk * (K + 1), ntask = nfull + (even ? (nblk >> 1) : 0);
     double tLam = 0.0, tLg = 0.0, tV = 0.0;
     long long slots = 0, inside = 0;
+    int k = warp / nblk, A = warp - k * nblk;                         // task t = warp, warp + nwarps, ...: k = t / n, A = t mod n
 #pragma unroll 1
-    for (int t = warp; t < ntask; t += nwarps) {
-        int k, A;
-        if (t < nfull) { k = t / nblk; A = t - k * nblk; }
-        else           { k = K + 1; A = t - nfull; }                 // even n: the offset n/2 once per block pair
+    for (;;) {
+        if (k > K && !(even && k == K + 1 && A < (nblk >> 1))) break;   // even n: the offset n/2 once per block pair
         const int i = (A << 5) + lane;
         const bool vi = i < N;
         const int32_t xi = x[i], yi = y[i], zi = z[i];
@@ -158,46 +170,44 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
         const int jb = B << 5;
         const bool diag = (k == 0);
         const bool bias = diag || (ragged && (A == nblk - 1 || B == nblk - 1));
-        long long gxi = 0, gyi = 0, gzi = 0, si = 0, gxj = 0, gyj = 0, gzj = 0, sj = 0;
-        const int nhalf = diag ? 1 : 2;
-        for (int hlf = 0; hlf < nhalf; ++hlf) {
-            SymAcc P;
-            P.gxi = P.gyi = P.gzi = P.si = P.gxj = P.gyj = P.gzj = P.sj = P.lam = P.lg = P.v = pk1(0.0f);
-            int n_in = 0;
-            const int s0 = diag ? 1 : 16 * hlf;
-            if (bias) sym_steps16<kEnergy, true>(x, y, z, jb, s0, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
-            else      sym_steps16<kEnergy, false>(x, y, z, jb, s0, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
-            slots += 16; inside += n_in;
-            si += fix_s(hsum2(P.si));
-            sj += fix_s(hsum2(P.sj));
-            if (kEnergy) {
-                gxi += fix_g(hsum2(P.gxi)); gyi += fix_g(hsum2(P.gyi)); gzi += fix_g(hsum2(P.gzi));
-                gxj += fix_g(hsum2(P.gxj)); gyj += fix_g(hsum2(P.gyj)); gzj += fix_g(hsum2(P.gzj));
-                tLam += (double)hsum2(P.lam);
-                tLg += (double)hsum2(P.lg);
-                tV += (double)hsum2(P.v);
-            }
+        SymAcc P;
+        P.gxi = P.gyi = P.gzi = P.si = P.gxj = P.gyj = P.gzj = P.sj = P.lam = P.lg = P.v = pk1(0.0f);
+        int n_in = 0;
+        const int s0 = diag ? 1 : 0, npk = diag ? 8 : 16;
+        if (bias) sym_steps<kEnergy, true>(x, y, z, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
+        else      sym_steps<kEnergy, false>(x, y, z, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
+        slots += 2 * npk; inside += n_in;
+        if (kEnergy) {
+            tLam += (double)hsum2(P.lam);
+            tLg += (double)hsum2(P.lg);
+            tV += (double)hsum2(P.v);
         }
         if (jb + lane < N) {
-            fix_add(ag + 3 * NP + jb + lane, sj);
+            fix_add(ag, 3 * NP + jb + lane, fix_s(hsum2(P.sj)));
             if (kEnergy) {
-                fix_add(ag + jb + lane, -gxj);                        // d_ji = -d_ij
-                fix_add(ag + NP + jb + lane, -gyj);
-                fix_add(ag + 2 * NP + jb + lane, -gzj);
+                fix_add(ag, jb + lane, -fix_g(hsum2(P.gxj)));         // d_ji = -d_ij
+                fix_add(ag, NP + jb + lane, -fix_g(hsum2(P.gyj)));
+                fix_add(ag, 2 * NP + jb + lane, -fix_g(hsum2(P.gzj)));
             }
         }
         if (vi) {
-            fix_add(ag + 3 * NP + i, si);
-            if (kEnergy) { fix_add(ag + i, gxi); fix_add(ag + NP + i, gyi); fix_add(ag + 2 * NP + i, gzi); }
+            fix_add(ag, 3 * NP + i, fix_s(hsum2(P.si)));
+            if (kEnergy) {
+                fix_add(ag, i, fix_g(hsum2(P.gxi)));
+                fix_add(ag, NP + i, fix_g(hsum2(P.gyi)));
+                fix_add(ag, 2 * NP + i, fix_g(hsum2(P.gzi)));
+            }
         }
+        A += nwarps;
+        while (A >= nblk) { A -= nblk; ++k; }
     }
     __syncthreads();
 
     double tG2 = 0.0;
     for (int i = tid; i < N; i += T) {
-        sv.S[(size_t)w * ld + i] = (double)ag[3 * NP + i] * (kSUnit / kFixS);      // R17: rebuild the running sum
+        sv.S[(size_t)w * ld + i] = fix_get(ag, 3 * NP + i) * (kSUnit / kFixS);     // R17: rebuild the running sum
         if (kEnergy) {
-            const double a = (double)ag[i] * (1.0 / kFixG), b = (double)ag[NP + i] * (1.0 / kFixG), c = (double)ag[2 * NP + i] * (1.0 / kFixG);
+            const double a = fix_get(ag, i) * (1.0 / kFixG), b = fix_get(ag, NP + i) * (1.0 / kFixG), c = fix_get(ag, 2 * NP + i) * (1.0 / kFixG);
             tG2 += a * a + b * b + c * c;
         }
     }

@@ -22,15 +22,10 @@
 // exactly 0 -- one DSETP on the fp64 pipe, the selects run on the integer pipe.
 #include "qmc_internal.h"
 
-#ifndef QMC_E64_UNROLL
-#define QMC_E64_UNROLL 1
-#endif
-
 namespace qmc {
 
 namespace {
 
-constexpr int kUnroll64 = QMC_E64_UNROLL;            // pair steps in flight per lane
 constexpr int kMaxOwn64 = 20;                        // i-blocks one warp can own (planner: ceil(nblk / nwarps) <= kMaxOwn64)
 
 struct Const64 {
@@ -78,7 +73,22 @@ __device__ __forceinline__ double exp_neg(double a)
     return __hiloint2double(__double2hiint(p) + (e << 20), __double2loint(p));
 }
 
-struct Pair64 { double mx, my, mz, t, gm, lt, v; bool in; };
+// HFD-B(HE) in two parts.  Every pair inside the cutoff adds its dispersion sum with F = 1 in straight-line code.
+// The two exponentials -- the repulsive term A exp(-alpha x + beta x^2), below 3e-15 of the dispersion term for
+// x = r/r_m >= 3 (8.9 A, i.e. for 97 % of the pairs inside the cutoff), and the damping F(x) - 1, which is 0 for
+// x >= D -- cost 19 fp64 instructions each in a dependent chain.  A pair with x < 3 (compared on the high word: kRepHi)
+// parks (x, D/x - 1, dispersion) in a per-lane pending slot; the exponentials are evaluated for all lanes that hold
+// an entry only when some lane is about to park a second one (about every 8th step), and once at the end.  Which
+// pairs are evaluated together depends on the data alone: reproducible.  This also leaves the pair arithmetic free
+// of branches, so that two pairs per lane are in flight (the kernel waits on fp64 latencies, not on the pipe).
+constexpr int kRepHi = 0x40080000;                   // high word of 3.0
+
+struct Pending64 {
+    double x = 3.0, q = 0.0, disp = 0.0, rep = 0.0, corr = 0.0;     // rep: sum of exp(..); corr: sum of (1 - F) disp
+    bool full = false;
+};
+
+struct Pair64 { double mx, my, mz, t, gm, lt, v, x, q, disp; bool in; };   // v = -dispersion sum: F = 1, no repulsive term (Pending64)
 
 // all terms of one pair; bias > 0 pushes the pair beyond the cutoff
 template <bool kEnergy>
@@ -99,7 +109,7 @@ __device__ __forceinline__ Pair64 pair64(double xi, double yi, double zi, double
     const double y4 = y2 * y2, z4 = z2 * z2;
     const double t = fma(z4, z, fma(y4, y, -C.sh));
     p.t = p.in ? t : 0.0;
-    p.gm = 0.0; p.lt = 0.0; p.v = 0.0;
+    p.gm = 0.0; p.lt = 0.0; p.v = 0.0; p.x = 0.0; p.q = 0.0; p.disp = 0.0;
     if (kEnergy) {
         const double y6 = y4 * y2, z6 = z4 * z2;
         const double y7 = y6 * y, z6y = z6 * y, z7 = z6 * z;
@@ -108,14 +118,10 @@ __device__ __forceinline__ Pair64 pair64(double xi, double yi, double zi, double
         const double x = r * C.inv_rm;
         const double w = C.rm2 * y2;                                // 1/x^2
         const double disp = w * w * w * fma(w, fma(w, C.c10, C.c8), C.c6);
-        double F = 1.0;
-        if (__any_sync(0xffffffffu, x < C.D)) {
-            const double q = fma(C.Drm, y, -1.0);                   // D/x - 1
-            const double e = exp_neg(-q * q);
-            F = x < C.D ? e : 1.0;
-        }
-        const double rep = C.A * exp_neg(x * fma(C.beta, x, -C.alpha));
-        p.v = p.in ? C.eps * fma(-F, disp, rep) : 0.0;
+        p.x = x;
+        p.q = fma(C.Drm, y, -1.0);                                  // D/x - 1
+        p.disp = disp;
+        p.v = p.in ? -disp : 0.0;
     }
     return p;
 }
@@ -125,8 +131,27 @@ __device__ __forceinline__ double shfl_from(double v, int src)
     return __hiloint2double(__shfl_sync(0xffffffffu, __double2hiint(v), src), __shfl_sync(0xffffffffu, __double2loint(v), src));
 }
 
+// evaluate the exponentials of every lane's pending entry (warp-uniform call)
+__device__ __forceinline__ void pending_flush(Pending64 &Q, const Const64 &C)
+{
+    const double e = exp_neg(Q.x * fma(C.beta, Q.x, -C.alpha));
+    Q.rep += Q.full ? e : 0.0;
+    const bool damped = Q.full && Q.x < C.D;
+    if (__any_sync(0xffffffffu, damped)) {
+        const double F = exp_neg(-Q.q * Q.q);
+        Q.corr += damped ? (1.0 - F) * Q.disp : 0.0;
+    }
+    Q.full = false;
+}
+__device__ __forceinline__ void pending_park(Pending64 &Q, const Pair64 &p, const Const64 &C)
+{
+    const bool hit = p.in && __double2hiint(p.x) < kRepHi;
+    if (__any_sync(0xffffffffu, hit && Q.full)) pending_flush(Q, C);
+    if (hit) { Q.x = p.x; Q.q = p.q; Q.disp = p.disp; Q.full = true; }
+}
+
 template <int T, bool kEnergy>
-__global__ void __launch_bounds__(T)
+__global__ void __launch_bounds__(T, (T <= 128 ? 4 : (T <= 256 ? 2 : 1)))
 energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -165,6 +190,7 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
     const int K = (nblk - 1) >> 1;                                    // full ring offsets
     const bool even = (nblk & 1) == 0;
     double tLam = 0.0, tV = 0.0;
+    Pending64 Q;
     double own[kMaxOwn64][4];                                         // G_x, G_y, G_z, S of this lane's particle in each own block
 #pragma unroll 1
     for (int a = 0; a < kMaxOwn64; ++a) { own[a][0] = 0.0; own[a][1] = 0.0; own[a][2] = 0.0; own[a][3] = 0.0; }
@@ -185,26 +211,30 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
             const bool vj = jb + lane < N;
             double gxj = 0.0, gyj = 0.0, gzj = 0.0, sj = 0.0;
             const int s0 = (k == 0) ? 1 : 0, s1 = (k == 0) ? 17 : 32;
-#pragma unroll kUnroll64
-            for (int s = s0; s < s1; ++s) {
-                const int src = (lane + s) & 31;
-                const bool ok = vi && (jb + src < N) && !(k == 0 && s == 16 && lane >= 16);
-                const Pair64 p = pair64<kEnergy>(xi, yi, zi, x[jb + src], y[jb + src], z[jb + src], ok ? 0.0 : kBig, C);
-                si += p.t;
-                double cx = 0.0, cy = 0.0, cz = 0.0;
-                if (kEnergy) {
-                    cx = p.gm * p.mx; cy = p.gm * p.my; cz = p.gm * p.mz;
-                    gxi += cx; gyi += cy; gzi += cz;
-                    tLam += p.lt;
-                    tV += p.v;
-                }
+#pragma unroll 1
+            for (int s = s0; s < s1; s += 2) {                        // two pairs per lane in flight (s1 - s0 is even)
+                const int srcA = (lane + s) & 31, srcB = (lane + s + 1) & 31;
+                const bool okA = vi && (jb + srcA < N);
+                const bool okB = vi && (jb + srcB < N) && !(k == 0 && s + 1 == 16 && lane >= 16);
+                const Pair64 pA = pair64<kEnergy>(xi, yi, zi, x[jb + srcA], y[jb + srcA], z[jb + srcA], okA ? 0.0 : kBig, C);
+                const Pair64 pB = pair64<kEnergy>(xi, yi, zi, x[jb + srcB], y[jb + srcB], z[jb + srcB], okB ? 0.0 : kBig, C);
+                si += pA.t;
+                si += pB.t;
                 // the lane that holds j = src gets this pair's terms: lane m receives from lane m - s
-                const int from = (lane - s) & 31;
-                sj += shfl_from(p.t, from);
+                const int fromA = (lane - s) & 31, fromB = (lane - s - 1) & 31;
+                sj += shfl_from(pA.t, fromA);
+                sj += shfl_from(pB.t, fromB);
                 if (kEnergy) {
-                    gxj -= shfl_from(cx, from);
-                    gyj -= shfl_from(cy, from);
-                    gzj -= shfl_from(cz, from);
+                    const double ax = pA.gm * pA.mx, ay = pA.gm * pA.my, az = pA.gm * pA.mz;
+                    const double bx = pB.gm * pB.mx, by = pB.gm * pB.my, bz = pB.gm * pB.mz;
+                    gxi += ax; gyi += ay; gzi += az;
+                    gxi += bx; gyi += by; gzi += bz;
+                    tLam += pA.lt; tLam += pB.lt;
+                    tV += pA.v; tV += pB.v;
+                    gxj -= shfl_from(ax, fromA); gyj -= shfl_from(ay, fromA); gzj -= shfl_from(az, fromA);
+                    gxj -= shfl_from(bx, fromB); gyj -= shfl_from(by, fromB); gzj -= shfl_from(bz, fromB);
+                    pending_park(Q, pA, C);
+                    pending_park(Q, pB, C);
                 }
             }
             if (vj) {
@@ -242,6 +272,8 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
         }
     }
     if (kEnergy) {
+        pending_flush(Q, C);
+        tV = C.eps * (fma(C.A, Q.rep, tV) + Q.corr);
         // each unordered pair was seen once: the Laplacian sum over i counts it twice
         tLam *= 2.0;
         tLam = warp_sum(tLam); tG2 = warp_sum(tG2); tV = warp_sum(tV);
@@ -296,7 +328,7 @@ int occupancy64(int smem)
 
 }  // namespace
 
-#define QMC_E64_THREADS(X) X(32) X(64) X(128) X(256) X(512)
+#define QMC_E64_THREADS(X) X(32) X(64) X(128) X(256) X(384) X(512)
 
 cudaError_t launch_energy_f64(qmc_ctx *c, double *d_out, bool energy)
 {
@@ -319,7 +351,7 @@ bool plan_energy_f64(qmc_ctx *c, EnergyPlan *out)
     while (2 * T < N && T < 256) T *= 2;
     if (g_tuning.energy_threads > 0) {
         const int v = g_tuning.energy_threads;
-        if (v >= 32 && v <= 512 && (v & (v - 1)) == 0) T = v;
+        if (v >= 32 && v <= 512 && ((v & (v - 1)) == 0 || v == 384)) T = v;
     }
     const int nblk = (N + 31) >> 5;
     while ((nblk + (T >> 5) - 1) / (T >> 5) > kMaxOwn64 && T < 512) T *= 2;     // own-block accumulators per warp
