@@ -481,7 +481,7 @@ extern "C" int qmc_pair_histogram(qmc_ctx *c, int32_t nbins, uint32_t *d_hist)
     if (!c || !d_hist) return QMC_E_ARG;
     if (!c->have_state) QMC_FAIL(c, QMC_E_STATE, "qmc_pair_histogram before qmc_init_walkers / qmc_set_positions");
     if (nbins < 1 || nbins > 8192) QMC_FAIL(c, QMC_E_ARG, "nbins = %d must lie in [1, 8192]", nbins);
-    if (3 * (long long)c->p.N * 8 + (long long)nbins * 4 > 227 * 1024)
+    if (!pair_histogram_fits(c->p.N, nbins, c->p.mode))
         QMC_FAIL(c, QMC_E_CAPACITY, "N = %d with %d bins does not fit the histogram kernel's shared memory", c->p.N, nbins);
     QMC_CUDA(c, launch_pair_histogram(c, nbins, d_hist));
     return QMC_OK;

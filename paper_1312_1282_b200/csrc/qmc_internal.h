@@ -102,6 +102,7 @@ cudaError_t launch_set_positions(qmc_ctx *c, const double *d_xyz);
 cudaError_t launch_get_positions(qmc_ctx *c, double *d_xyz);
 cudaError_t launch_acceptance(qmc_ctx *c, double *d_out);
 cudaError_t launch_pair_histogram(qmc_ctx *c, int nbins, uint32_t *d_hist);   // qmc_observables.cu
+bool pair_histogram_fits(int N, int nbins, int mode);                        // shared-memory capacity of that kernel
 bool plan_sweep(qmc_ctx *c, SweepPlan *out);
 bool plan_energy(qmc_ctx *c, EnergyPlan *out);
 cudaError_t launch_energy_f32(qmc_ctx *c, double *d_out, bool energy);

@@ -607,7 +607,8 @@ def test_local_energy_fp64_ordered_fallback(qmc, oracle, tuning):
 
 # ------------------------------------------------------------------------------ pair distribution function
 @pytest.mark.parametrize("mode_name,N,nb", [("fp64", 2, 7), ("fp64", 100, 64), ("fp64", 515, 200), ("fp32c", 256, 128),
-                                            ("fp64", 1952, 512), ("fp32c", 1952, 512)])
+                                            ("fp64", 1952, 512), ("fp32c", 1952, 512),
+                                            ("fp64", 300, 1000), ("fp32c", 300, 1000)])      # > 512 bins: unfiltered kernel
 def test_pair_histogram_bit_exact(qmc, oracle, mode_name, N, nb):
     """qmc_pair_histogram (NEXT-2) against the oracle on the configuration the GPU holds after a
     few sweeps: integer counts, bit-exact (the bin arithmetic is specified to the bit)."""
@@ -623,6 +624,27 @@ def test_pair_histogram_bit_exact(qmc, oracle, mode_name, N, nb):
     assert Hg.sum() > 0 or N == 2
     with pytest.raises(qmc.QmcError):
         q.pair_histogram(0)
+
+
+@pytest.mark.parametrize("mode_name", ["fp64", "fp32c"])
+def test_pair_histogram_distances_on_bin_edges(qmc, oracle, mode_name):
+    """The filtered histogram kernel (fp32 estimate, exact fp64 arithmetic only near a bin edge or the cutoff) on a
+    configuration made of bin edges: a simple cubic lattice of 8^3 points with spacing L/8 and 64 bins of width L/128,
+    so that every distance along an axis is a whole number of bins and the face diagonals sit on the cutoff's side of
+    rounding.  The guard band must send all of them to the specified arithmetic: counts equal the oracle's."""
+    mode = qmc.QMC_FP64 if mode_name == "fp64" else qmc.QMC_FP32C
+    N, W, nb = 512, 2, 64
+    q, L = make(qmc, N, W, mode)
+    g = np.arange(8) * (L / 8.0)
+    X, Y, Z = np.meshgrid(g, g, g, indexing="ij")
+    lat = np.stack([X.ravel(), Y.ravel(), Z.ravel()])                       # [3][N]
+    xyz = np.stack([lat, (lat + L / 16.0) % L])                            # second walker: the lattice shifted by half a cell
+    q.set_positions(xyz)
+    xyz = q.get_positions().cpu().numpy()                                   # what the GPU holds (FP32C: on the grid)
+    Hg = q.pair_histogram(nb).cpu().numpy()
+    Ho = oracle.pair_histogram(orc_sys(oracle, N, L), xyz, nb)
+    assert np.array_equal(Hg.astype(np.int64), Ho.astype(np.int64))
+    assert Hg.sum() > 0
 
 
 # ------------------------------------------------------------------------------ boundary behaviour
