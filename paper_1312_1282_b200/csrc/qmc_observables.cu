@@ -79,6 +79,7 @@ __device__ __forceinline__ int32_t fix_coord(double x, double invL)
 }
 
 struct HistCtx {
+    uint32_t Hs;                    // shared-window byte address of the bins, biased (see hist_pair)
     uint32_t *H, *Q;                // bins; this warp's queue of pairs for the specified arithmetic (i << 16 | j)
     int cnt;                        // entries in the queue (warp-uniform)
     float uscale, lo_off, hi_off;
@@ -102,7 +103,10 @@ __device__ __forceinline__ bool hist_pair(const HistCtx &C, int32_t xi, int32_t 
     bool slow = b0 != b1;                                             // near a bin edge or the cutoff
     if (kMask) slow = slow && valid;
     const bool count = kMask ? (valid && !slow && b1 < C.in_limit) : (!slow && b1 < C.in_limit);
-    if (count) atomicAdd(C.H + (b1 - 0x4B000000), 1u);
+    // predicated reduction instead of a branch around atomicAdd (the branch costs BSSY / BRA / BSYNC per pair);
+    // Hs = shared-window address of bin 0 minus 4 x 0x4B000000
+    asm volatile("{ .reg .pred p; setp.ne.s32 p, %2, 0; @p red.shared.add.u32 [%0], %1; }"
+                 :: "r"(C.Hs + 4u * (uint32_t)b1), "r"(1u), "r"((int)count) : "memory");
     return slow;
 }
 __device__ __forceinline__ void hist_enqueue(HistCtx &C, bool slow, int i, int j, int lane)
@@ -146,6 +150,7 @@ __global__ void __launch_bounds__(256, 4) pair_histogram_kernel(StateView sv, in
     const double inv_dr = __ddiv_rn((double)nbins, h);
     HistCtx C;
     C.H = H; C.Q = Qall + warp * kQueue; C.cnt = 0;
+    C.Hs = (uint32_t)__cvta_generic_to_shared(H) - 4u * 0x4B000000u;
     C.uscale = (float)nbins * 0x1p-31f;                               // u = (r / L) 2 nbins, r / L arrives times 2^32
     // floor(v) for 0 <= v < 2^22 not within rounding of an integer: the low bits of fl((v - 1/2) + 2^23)
     C.lo_off = -(0.5f + kGuard); C.hi_off = -(0.5f - kGuard);
