@@ -147,6 +147,13 @@ __device__ __forceinline__ double rsqrt_pos(double x)
     const double q = y * e;
     return fma(q, p, y);                       // y (1 + e/2 + 3 e^2/8)
 }
+// a < b for a >= 0 or NaN, b > 0: the same answer as the fp64 comparison (the bit patterns of non-negative doubles
+// order like integers, NaN -- the poison of the sweep kernel -- lies above every number), taken on the integer
+// pipe, which idles in fp64 mode, instead of a DSETP on the fp64 pipe that bounds it
+__device__ __forceinline__ bool less_pos(double a, double b)
+{
+    return (unsigned long long)__double_as_longlong(a) < (unsigned long long)__double_as_longlong(b);      // unsigned: a NaN of either sign is large
+}
 // 1/x for the z = 1/(L - r) terms: second order, relative error e^2 < 1e-12 on terms that make up 1e-3 of the pair
 // sums and vanish against y^5 where a trial overlaps a neighbour
 __device__ __forceinline__ double rcp_pos(double x)

@@ -100,7 +100,7 @@ __device__ __forceinline__ Pair64 pair64(double xi, double yi, double zi, double
     p.my = min_image(yi, ys, C.h);
     p.mz = min_image(zi, zs, C.h);
     const double r2 = fma(p.mz, p.mz, fma(p.my, p.my, fma(p.mx, p.mx, bias)));
-    p.in = r2 < C.h2;
+    p.in = less_pos(r2, C.h2);
     const double r2c = p.in ? r2 : C.h2;
     const double y = rsqrt_pos(r2c);
     const double r = r2c * y;
