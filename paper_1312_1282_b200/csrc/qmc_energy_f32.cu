@@ -45,7 +45,7 @@ __device__ __forceinline__ void tile16(const int32_t *__restrict__ x, const int3
 {
     Acc32 P;
     P.gx = P.gy = P.gz = P.lam = P.s = P.v = pk1(0.0f);
-#pragma unroll 1
+#pragma unroll 4
     for (int g = 0; g < 4; ++g) {
         // kGlobal: the coordinates stream from global memory through the read-only path (all lanes read the same
         // address; the L1 serves the other warps of the block)

@@ -62,7 +62,7 @@ __device__ __forceinline__ void sym_steps(const int32_t *__restrict__ x, const i
                                             int32_t xi, int32_t yi, int32_t zi, const AzizF32 &E, int32_t zero,
                                             SymAcc &P, int &n_in)
 {
-#pragma unroll 2
+#pragma unroll 4
     for (int p = 0; p < npk; ++p) {
         const int sa = s0 + 2 * p, sb = sa + 1;
         const int ja = (lane + sa) & 31, jl = (lane + sb) & 31;
