@@ -306,6 +306,27 @@ def test_local_energy_fp32c(qmc, oracle, tuning, N, variant):
     assert np.abs(S[0] - Sr).max() < 2e-6 * np.abs(Sr).max()
 
 
+@pytest.mark.parametrize("mode_name,N", [("fp32c", 1952), ("fp64", 1952), ("fp32c", 300), ("fp64", 515)])
+def test_local_energy_reproducible_to_the_bit(qmc, mode_name, N):
+    """The unordered-pair energy kernels merge per-particle sums of many warps (FP32C: fixed-point integer atomics in
+    any order of arrival; FP64: a fixed order behind barriers).  The same configuration must give the same bits on
+    every launch and wherever the walker sits in the launch (S_i feeds the next sweep's decisions)."""
+    import torch
+    mode = qmc.QMC_FP64 if mode_name == "fp64" else qmc.QMC_FP32C
+    q, L = make(qmc, N, 40, mode)
+    q.init_walkers(11)
+    q.sweep(2, 1.0)
+    x = q.get_positions()
+    e0, S0 = q.local_energy().clone(), q.pair_sums().clone()
+    for _ in range(3):
+        assert torch.equal(q.local_energy(), e0)
+        assert torch.equal(q.pair_sums(), S0)
+    q2, _ = make(qmc, N, 7, mode)
+    q2.set_positions(x[20:27].cpu().numpy())
+    assert torch.equal(q2.local_energy(), e0[20:27])
+    assert torch.equal(q2.pair_sums(), S0[20:27])
+
+
 @pytest.mark.parametrize("N,W", [(64, 16), (256, 4)])
 def test_local_energy_fp32c_equilibrated_liquid(qmc, oracle, N, W):
     """The regime the tolerance is hardest in: an EQUILIBRATED liquid (E = V + T cancels ~3.5x).  The
