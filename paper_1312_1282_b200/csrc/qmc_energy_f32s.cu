@@ -57,7 +57,7 @@ struct SymAcc {            // fp32 partial sums of up to 16 packed steps
 // npk = 16, s0 = 0 for a full block pair, npk = 8, s0 = 1 for the diagonal block.
 //   kBias: some slots must be forced beyond the cutoff (padding particles, second half of diagonal step 16)
 template <bool kEnergy, bool kBias>
-__device__ __forceinline__ void sym_steps(const int32_t *__restrict__ x, const int32_t *__restrict__ y, const int32_t *__restrict__ z,
+__device__ __forceinline__ void sym_steps(const int4 *__restrict__ xyz,
                                             int jb, int s0, int npk, int lane, bool vi, int N, bool diag,
                                             int32_t xi, int32_t yi, int32_t zi, const AzizF32 &E, int32_t zero,
                                             SymAcc &P, int &n_in)
@@ -72,7 +72,8 @@ __device__ __forceinline__ void sym_steps(const int32_t *__restrict__ x, const i
             const bool okb = vi && (jb + jl < N) && !(diag && sb == 16 && lane >= 16);
             bias2 = pk2(oka ? 0.0f : 0x1p63f, okb ? 0.0f : 0x1p63f);
         }
-        const Pair2 q = pair_geom(xi, yi, zi, x[jb + ja], x[jb + jl], y[jb + ja], y[jb + jl], z[jb + ja], z[jb + jl], bias2, zero);
+        const int4 ca = xyz[jb + ja], cb = xyz[jb + jl];             // one 16-byte read per particle
+        const Pair2 q = pair_geom(xi, yi, zi, ca.x, cb.x, ca.y, cb.y, ca.z, cb.z, bias2, zero);
         n_in += (__float_as_int(q.a) < kClampBits ? 1 : 0) + (__float_as_int(q.b) < kClampBits ? 1 : 0);
         const f32x2 t = pair_t(q);
         P.si = add2(P.si, t);
@@ -117,8 +118,7 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
     double  *red = reinterpret_cast<double *>(smem_raw);              // [3][32]
                                                                       // red[97]: opaque zero
     int32_t *ag = reinterpret_cast<int32_t *>(red + 98);              // [4][NP][2]: G_x, G_y, G_z, S as fixed point (hi, lo)
-    int32_t *x   = ag + 8 * NP;                                       // [3][NP]
-    int32_t *y = x + NP, *z = x + 2 * NP;
+    int4 *xyz = reinterpret_cast<int4 *>(ag + 8 * NP);                // [NP]: fixed-point x, y, z of a particle in one 16-byte word
 
     const GroupDev g = sv.groups[sv.group_of[w]];
     AzizF32 E;
@@ -127,9 +127,7 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
     const float *gpos = reinterpret_cast<const float *>(sv.pos) + (size_t)w * 3 * ld;
     for (int j = tid; j < NP; j += T) {
         const bool in = j < N;
-        x[j] = in ? enc_coord(gpos[j]) : 0;
-        y[j] = in ? enc_coord(gpos[ld + j]) : 0;
-        z[j] = in ? enc_coord(gpos[2 * ld + j]) : 0;
+        xyz[j] = in ? make_int4(enc_coord(gpos[j]), enc_coord(gpos[ld + j]), enc_coord(gpos[2 * ld + j]), 0) : make_int4(0, 0, 0, 0);
         *reinterpret_cast<int2 *>(ag + 2 * j) = make_int2(0, 0);
         *reinterpret_cast<int2 *>(ag + 2 * (NP + j)) = make_int2(0, 0);
         *reinterpret_cast<int2 *>(ag + 2 * (2 * NP + j)) = make_int2(0, 0);
@@ -164,7 +162,8 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
         if (k > K && !(even && k == K + 1 && A < (nblk >> 1))) break;   // even n: the offset n/2 once per block pair
         const int i = (A << 5) + lane;
         const bool vi = i < N;
-        const int32_t xi = x[i], yi = y[i], zi = z[i];
+        const int4 ci = xyz[i];
+        const int32_t xi = ci.x, yi = ci.y, zi = ci.z;
         int B = A + k;
         if (B >= nblk) B -= nblk;
         const int jb = B << 5;
@@ -174,8 +173,8 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
         P.gxi = P.gyi = P.gzi = P.si = P.gxj = P.gyj = P.gzj = P.sj = P.lam = P.lg = P.v = pk1(0.0f);
         int n_in = 0;
         const int s0 = diag ? 1 : 0, npk = diag ? 8 : 16;
-        if (bias) sym_steps<kEnergy, true>(x, y, z, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
-        else      sym_steps<kEnergy, false>(x, y, z, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
+        if (bias) sym_steps<kEnergy, true>(xyz, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
+        else      sym_steps<kEnergy, false>(xyz, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
         slots += 2 * npk; inside += n_in;
         if (kEnergy) {
             tLam += (double)hsum2(P.lam);
@@ -236,7 +235,7 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
     }
 }
 
-int smem_bytes32s(int N) { const int NP = ((N + 31) >> 5) << 5; return 98 * 8 + 4 * NP * 8 + 3 * NP * 4; }
+int smem_bytes32s(int N) { const int NP = ((N + 31) >> 5) << 5; return 98 * 8 + 4 * NP * 8 + 4 * NP * 4; }
 
 template <int T>
 cudaError_t launch32s(qmc_ctx *c, double *d_out, bool energy)
