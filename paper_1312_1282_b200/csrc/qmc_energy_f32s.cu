@@ -60,7 +60,7 @@ template <bool kEnergy, bool kBias>
 __device__ __forceinline__ void sym_steps(const int4 *__restrict__ xyz,
                                             int jb, int s0, int npk, int lane, bool vi, int N, bool diag,
                                             int32_t xi, int32_t yi, int32_t zi, const AzizF32 &E, int32_t zero,
-                                            SymAcc &P, int &n_in)
+                                            SymAcc &P, f32x2 &n_out2)
 {
 #pragma unroll 4
     for (int p = 0; p < npk; ++p) {
@@ -74,13 +74,15 @@ __device__ __forceinline__ void sym_steps(const int4 *__restrict__ xyz,
         }
         const int4 ca = xyz[jb + ja], cb = xyz[jb + jl];             // one 16-byte read per particle
         const Pair2 q = pair_geom(xi, yi, zi, ca.x, cb.x, ca.y, cb.y, ca.z, cb.z, bias2, zero);
-        n_in += (__float_as_int(q.a) < kClampBits ? 1 : 0) + (__float_as_int(q.b) < kClampBits ? 1 : 0);
+        // clamped slots are counted in fp32 (exact far beyond the ~1e4 slots a thread sees): two compares that write
+        // 1.0f / 0.0f and one packed add instead of compare + predicated integer add per slot
+        if (kEnergy) n_out2 = add2(n_out2, pk2(q.a < 1.0f ? 0.0f : 1.0f, q.b < 1.0f ? 0.0f : 1.0f));
         const f32x2 t = pair_t(q);
         P.si = add2(P.si, t);
         float t0, t1;
         upk2(t, t0, t1);
         // lane m holds j = m: it receives the first pair's terms from lane m - sa, the second's from m - sb
-        const int fa = (lane - sa) & 31, fb = (lane - sb) & 31;
+        const int fa = lane - sa, fb = lane - sb;                    // shfl takes the source lane modulo 32
         P.sj = add2(P.sj, pk2(shfl_f(t0, fa), shfl_f(t1, fb)));
         if (kEnergy) {
             // gm = (y^6 - z^6) y;  Laplacian term 2 y^7 + 3 z^7 + z^6 y = 3 (y^7 + z^7) - gm: the two sums are kept apart
@@ -155,7 +157,7 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
     const int K = (nblk - 1) >> 1;
     const bool even = (nblk & 1) == 0, ragged = (N & 31) != 0;
     double tLam = 0.0, tLg = 0.0, tV = 0.0;
-    long long slots = 0, inside = 0;
+    f32x2 n_out2 = pk1(0.0f);                                         // clamped slots, per packed lane
     int k = warp / nblk, A = warp - k * nblk;                         // task t = warp, warp + nwarps, ...: k = t / n, A = t mod n
 #pragma unroll 1
     for (;;) {
@@ -171,11 +173,9 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
         const bool bias = diag || (ragged && (A == nblk - 1 || B == nblk - 1));
         SymAcc P;
         P.gxi = P.gyi = P.gzi = P.si = P.gxj = P.gyj = P.gzj = P.sj = P.lam = P.lg = P.v = pk1(0.0f);
-        int n_in = 0;
         const int s0 = diag ? 1 : 0, npk = diag ? 8 : 16;
-        if (bias) sym_steps<kEnergy, true>(xyz, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
-        else      sym_steps<kEnergy, false>(xyz, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_in);
-        slots += 2 * npk; inside += n_in;
+        if (bias) sym_steps<kEnergy, true>(xyz, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_out2);
+        else      sym_steps<kEnergy, false>(xyz, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_out2);
         if (kEnergy) {
             tLam += (double)hsum2(P.lam);
             tLg += (double)hsum2(P.lg);
@@ -211,7 +211,7 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
         }
     }
     if (kEnergy) {
-        const double n_out = (double)(slots - inside);
+        const double n_out = (double)hsum2(n_out2);
         tLam = 2.0 * (3.0 * (tLam - 2.0 * n_out) - tLg);              // each unordered pair seen once; a clamped slot adds y^7 + z^7 = 2, gm = 0
         tV -= (double)KV * n_out;
         tLam = warp_sum(tLam); tG2 = warp_sum(tG2); tV = warp_sum(tV);

@@ -233,7 +233,7 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
                     si += pA.t;
                     si += pB.t;
                     // the lane that holds j = src gets this pair's terms: lane m receives from lane m - s
-                    const int fromA = (lane - s) & 31, fromB = (lane - s - 1) & 31;
+                    const int fromA = lane - s, fromB = lane - s - 1;     // shfl takes the source lane modulo 32
                     sj += shfl_from(pA.t, fromA);
                     sj += shfl_from(pB.t, fromB);
                     if (kEnergy) {
@@ -262,7 +262,7 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
                         tLam += p.lt;
                         tV += p.v;
                     }
-                    const int from = (lane - s) & 31;                 // lane m receives from lane m - s
+                    const int from = lane - s;                        // lane m receives from lane m - s (modulo 32)
                     sj += shfl_from(p.t, from);
                     if (kEnergy) {
                         gxj -= shfl_from(cx, from);
