@@ -101,7 +101,9 @@ int qmc_local_energy(qmc_ctx *c, double *d_out);
  * function g(r) (l.421, l.468): d_hist device [W][nbins] uint32, bin k counts the
  * pairs i < j with minimum-image distance r in [k, k+1) * (L/2)/nbins; pairs with r >= L/2 are not counted.
  * The bin of a pair is specified to the bit, so counts are reproducible exactly.
- * 1 <= nbins <= 8192; QMC_E_CAPACITY if 24 N + 4 nbins bytes exceed one CTA's shared memory. */
+ * Up to 512 bins the kernel decides most pairs from an fp32 estimate and evaluates the specified fp64 arithmetic only
+ * near a bin edge (same counts); more bins take the fp64 arithmetic for every pair.
+ * 1 <= nbins <= 8192; QMC_E_CAPACITY if 12 N + 4 nbins + 5 KB exceed one CTA's shared memory (N <= ~18 000). */
 int qmc_pair_histogram(qmc_ctx *c, int32_t nbins, uint32_t *d_hist);
 
 /* d_out: device [W] accepted / attempted moves since qmc_init_walkers / qmc_set_positions. */
