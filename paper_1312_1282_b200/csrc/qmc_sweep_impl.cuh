@@ -71,7 +71,7 @@ __device__ __forceinline__ double pair_t(double px, double py, double pz, double
     const double y2 = y * y, z2 = z * z;
     const double y4 = y2 * y2, z4 = z2 * z2;
     const double t = fma(z4, z, fma(y4, y, -P.sh));
-    return less_pos(r2, P.h2) ? t : 0.0;
+    return r2 < P.h2 ? t : 0.0;
 }
 // FP32C: wrapping integer difference = minimum image * 2^32; r^2 is clamped to h^2 = 1/4, where
 // y = z = 2 and t = 16*2 + (16*2 - 64) = 0 exactly, so pairs at and beyond the cutoff add exactly 0.
