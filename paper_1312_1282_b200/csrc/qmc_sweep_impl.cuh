@@ -92,19 +92,26 @@ __device__ __forceinline__ float pair_t(int32_t px, int32_t py, int32_t pz, int3
     return fmaf(z4, z, fmaf(y4, y, -64.0f));
 }
 
-// Two FP32C pair terms at once, in units of 32: returns t/32 = (y/2)^5 + (z/2)^5 - 2.
-// r^2 arrives as d^2 2^64 (integer differences); ONE integer instruction (VIADDMNMX: add to the exponent
-// field, then min) rescales it by 2^-62 and clamps it: a4 = min(4 r^2, 1).  Then yh = rsqrt(a4) = y/2,
-// q = a4 yh = 2r, w = 2 - q = 2(1 - r), zh = 1/w = z/2; at the clamp yh = zh = 1 and t/32 = 0 exactly.
-// bias2 holds 0 or 2^63 per lane (padding: clamps).  Every scale factor is a power of two (and an even one
-// in front of the reciprocal square root), so 32 x the result is bit-identical to the scalar form; the
-// packed kernels keep their sums in these units (kT2Unit) and convert on load / store.
-// d != 0 means d^2 2^64 >= 1, so the exponent subtraction cannot underflow; d = 0 (two particles on one grid
-// point) gives a negative number, rsqrt = NaN, and the move is rejected as it was with y = inf.
-constexpr double kT2Unit = 32.0;
+// Two FP32C pair terms at once.  r^2 arrives as d^2 2^64 (integer differences); ONE integer instruction (VIADDMNMX:
+// add to the exponent field, then min) rescales it by 2^-64 and clamps it: a = min(r^2, 1/4).  With a + b = 1 one has
+// a^-5 + b^-5 = (1 - 5ab + 5 (ab)^2) / (ab)^5, so with r = sqrt(a), p = r (1 - r) = r - r^2 and w = 1/p
+//   t = y^5 + z^5 - 64 = w^3 (w^2 - 5w + 5) - 64:
+// one square root, one reciprocal and SIX packed multiply-adds (the form with y = 1/r and z = 1/(1-r) separately takes
+// eight).  At the clamp r = 1/2, p = 1/4, w = 4 and t = 64 (16 - 20 + 5) - 64 = 0 exactly (MUFU.SQRT and MUFU.RCP are
+// exact on powers of two; tests/test_gpu_parity.py checks the zero through the padding slots).  bias2 holds 0 or 2^63
+// per lane (padding: clamps).  d = 0 (two particles on one grid point) gives a negative number, sqrt = NaN, and the
+// move is rejected.  Relative error of a term ~5e-7 near contact, absolute error ~2e-5 near the cutoff (where t -> 0
+// quadratically): inside the R23 budget.
+constexpr double kT2Unit = 1.0;
 __device__ __forceinline__ float scale_clamp_r2(float a)
 {
-    return __int_as_float(__viaddmin_s32(__float_as_int(a), -(62 << 23), 0x3F800000));
+    return __int_as_float(__viaddmin_s32(__float_as_int(a), -(64 << 23), 0x3E800000));      // min(a 2^-64, 1/4)
+}
+__device__ __forceinline__ float sqrt_pos(float x)
+{
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
 }
 __device__ __forceinline__ f32x2 pair_t2(int32_t px, int32_t py, int32_t pz, int32_t X0, int32_t X1, int32_t Y0, int32_t Y1,
                                          int32_t Z0, int32_t Z1, f32x2 bias2, int32_t zero)
@@ -117,15 +124,14 @@ __device__ __forceinline__ f32x2 pair_t2(int32_t px, int32_t py, int32_t pz, int
     upk2(r2p, a, b);
     a = scale_clamp_r2(a);
     b = scale_clamp_r2(b);
-    const f32x2 y = pk2(rsqrt_pos(a), rsqrt_pos(b));                    // y/2
-    const f32x2 q = mul2(pk2(a, b), y);                                 // 2r
-    const f32x2 w = fma2(q, pk2(-1.0f, -1.0f), pk2(2.0f, 2.0f));
-    float wa, wb;
-    upk2(w, wa, wb);
-    const f32x2 z = pk2(rcp_pos(wa), rcp_pos(wb));                      // z/2
-    const f32x2 y2 = mul2(y, y), z2 = mul2(z, z);
-    const f32x2 y4 = mul2(y2, y2), z4 = mul2(z2, z2);
-    return fma2(z4, z, fma2(y4, y, pk2(-2.0f, -2.0f)));
+    const f32x2 r = pk2(sqrt_pos(a), sqrt_pos(b));
+    const f32x2 p = sub2(r, pk2(a, b));                                 // r - r^2 = r (1 - r)
+    float pa, pb;
+    upk2(p, pa, pb);
+    const f32x2 w = pk2(rcp_pos(pa), rcp_pos(pb));
+    const f32x2 w2 = mul2(w, w), w3 = mul2(w2, w);
+    const f32x2 u = fma2(w, w, fma2(w, pk2(-5.0f, -5.0f), pk2(5.0f, 5.0f)));
+    return fma2(w3, u, pk2(-64.0f, -64.0f));
 }
 
 template <typename Real> __device__ __forceinline__ typename ModeT<Real>::Coord poison_of(typename ModeT<Real>::Coord p);
