@@ -8,6 +8,7 @@
 #include <nvtx3/nvToolsExt.h>          // header-only NVTX v3: ranges around the hot launches
 
 #include "qmc_internal.h"
+#include "qmc_energy_f32_pair.cuh"     // aziz_f32_scale (host)
 
 using namespace qmc;
 
@@ -309,6 +310,7 @@ extern "C" int qmc_create(const qmc_params *p, void *cuda_stream, void *d_state,
         G.az.eps = a[0]; G.az.inv_rm = 1.0 / rm; G.az.rm2 = rm * rm; G.az.A = a[2];
         G.az.alpha = a[3]; G.az.beta = a[4]; G.az.c6 = a[5]; G.az.c8 = a[6]; G.az.c10 = a[7];
         G.az.D = a[8]; G.az.Drm = a[8] * rm;
+        G.az.f32_scale = (p->mode == QMC_FP64) ? 1.0 : e32::aziz_f32_scale(G.az);
     }
 
     // state buffer

@@ -22,6 +22,7 @@ namespace qmc {
 // so coordinate differences and the minimum-image fold are EXACT in fp32.
 struct AzizDev {            // HFD-B(HE), l.131, R3; inv_rm, rm2, Drm in coordinate units
     double eps, inv_rm, rm2, A, alpha, beta, c6, c8, c10, D, Drm;
+    double f32_scale;       // FP32C: the potential is summed in units of this number of kelvin (qmc_energy_f32_pair.cuh)
 };
 
 struct GroupDev {

@@ -193,7 +193,8 @@ energy32_kernel(StateView sv, double Dk, double *__restrict__ out)
                 const double T_PB = -Dku * (lam + g2);
                 const double T_JF = -0.5 * Dku * lam;
                 double *o = out + (size_t)w * 4;
-                o[0] = c + T_PB; o[1] = c; o[2] = T_PB; o[3] = T_JF;
+                const double V = c * g.az.f32_scale;                                     // the potential was summed in units of f32_scale K
+                o[0] = V + T_PB; o[1] = V; o[2] = T_PB; o[3] = T_JF;
             }
         }
     }
@@ -310,7 +311,8 @@ __global__ void finalize32g_kernel(StateView sv, double Dk, const double *__rest
     const double T_PB = -Dku * (lam + g2);
     const double T_JF = -0.5 * Dku * lam;
     double *o = out + (size_t)w * 4;
-    o[0] = c + T_PB; o[1] = c; o[2] = T_PB; o[3] = T_JF;
+    const double V = c * g.az.f32_scale;                                     // the potential was summed in units of f32_scale K
+                o[0] = V + T_PB; o[1] = V; o[2] = T_PB; o[3] = T_JF;
 }
 
 int smem_bytes32(int N) { return 96 * 8 + 3 * (((N + 31) >> 5) << 5) * 4; }

@@ -18,6 +18,29 @@ namespace e32 {
 constexpr int    kClampBits = 0x3F800000;      // bit pattern of 1.0f = the clamped a4; inside the cutoff iff bits(a4) < this
 constexpr double kSUnit = 32.0, kGUnit = 128.0, kLamClamp = 6.0;
 
+// The four amplitudes (eps A and the three dispersion coefficients) are single fp32 numbers; their rounding errors
+// (up to 6e-8 each) are systematic, and the repulsive and the dispersion sums are each several times |V|, so they showed
+// as +0.5 ... 2e-6 on V.  The potential is therefore summed in units of s kelvin, with s in [1, 2) searched on the host
+// (aziz_f32_scale, once per qmc_create) such that all four amplitudes divided by s round to fp32 with a relative
+// error below ~5e-9; the total is multiplied by s in fp64 at the end.
+inline double aziz_f32_scale(const AzizDev &a)
+{
+    const double r2 = a.rm2, r6 = r2 * r2 * r2;
+    const double c[4] = {a.eps * a.A, a.eps * a.c6 * r6 * 64.0, a.eps * a.c8 * r6 * r2 * 256.0, a.eps * a.c10 * r6 * r2 * r2 * 1024.0};
+    double best = 1.0, best_err = 1e300;
+    for (int i = 0; i < 400000; ++i) {
+        const double s = 1.0 + (double)i * 2.5e-6;
+        double err = 0.0;
+        for (int k = 0; k < 4; ++k) {
+            const double v = c[k] / s;
+            const double e = fabs((double)(float)v / v - 1.0);
+            err = e > err ? e : err;
+        }
+        if (err < best_err) { best_err = err; best = s; }
+    }
+    return best;
+}
+
 // HFD-B(HE) constants for packed fp32 evaluation.  Every constant that multiplies into the steep
 // repulsive exponential or the dispersion sum is folded (in fp64, on load) into ONE rounded coefficient
 // or carried as hi + lo, so that no fp32 rounding of a CONSTANT puts a systematic relative error on
@@ -37,13 +60,14 @@ struct AzizF32 {
         };
         split(-0.5 * a.alpha * a.inv_rm * log2e, a1h, a1l);
         split(0.25 * a.beta * a.inv_rm * a.inv_rm * log2e, a2h, a2l);
-        const float eA = (float)(a.eps * a.A);
+        const double is = 1.0 / a.f32_scale;                         // see aziz_f32_scale()
+        const float eA = (float)(a.eps * a.A * is);
         epsA = pk1(eA);
         epsAln2 = pk1((float)((double)eA * ln2));
         const double r2 = a.rm2, r6 = r2 * r2 * r2;
-        nk6 = pk1((float)(-a.eps * a.c6 * r6 * 64.0));
-        nk8 = pk1((float)(-a.eps * a.c8 * r6 * r2 * 256.0));
-        nk10 = pk1((float)(-a.eps * a.c10 * r6 * r2 * r2 * 1024.0));
+        nk6 = pk1((float)(-a.eps * a.c6 * r6 * 64.0 * is));
+        nk8 = pk1((float)(-a.eps * a.c8 * r6 * r2 * 256.0 * is));
+        nk10 = pk1((float)(-a.eps * a.c10 * r6 * r2 * r2 * 1024.0 * is));
         split(2.0 * a.Drm * sl, Dh, Dl);
         nDc = pk1((float)(-sl));
     }
@@ -90,14 +114,18 @@ __device__ __forceinline__ Pair2 pair_geom(int32_t xi, int32_t yi, int32_t zi, i
 // t/32 = yh^5 + zh^5 - 2 (raw pair-sum term t = y^5 + z^5 - 64, u = c1 t); exactly 0 at the clamp
 __device__ __forceinline__ f32x2 pair_t(const Pair2 &p) { return fma2(p.z4, p.z, fma2(p.y4, p.y, pk1(-2.0f))); }
 
-// HFD-B(HE) of the two pairs in K.  The hardware rsqrt is first refined by one Newton step,
-// Y = yh f with f = 3/2 - q yh / 2 (the seed is good to ~2^-22 and the repulsive exponential
-// amplifies a relative error of r ~11x); R = q f = 2r.
+// HFD-B(HE) of the two pairs in K (in units of f32_scale K).  The hardware rsqrt is first refined by one Newton step
+// (the seed is good to ~2^-22 and the repulsive exponential amplifies a relative error of r ~11x), written as
+//   c = 1/2 - q yh / 2 (one FMA: the small correction keeps its full relative precision),  Y = yh + yh c,  R = q + q c.
+// The form Y = yh f with f = 3/2 - q yh / 2 costs the same four instructions but rounds f on the fp32 grid around 1
+// (spacing 6e-8 below, 1.2e-7 above): measured mean errors -1.5e-8 on Y and -1.0e-8 on R, i.e. -9e-8 on Y^6 and
+// +1.4e-7 on the repulsive term -- the +0.5 ... 2e-6 systematic error V used to carry, since the two sums are each
+// several times |V|.  With c the means are < 4e-10.
 __device__ __forceinline__ f32x2 aziz2(const Pair2 &p, const AzizF32 &E)
 {
-    const f32x2 f = fma2(p.q, mul2(p.y, pk1(-0.5f)), pk1(1.5f));
-    const f32x2 y = mul2(p.y, f);
-    const f32x2 r = mul2(p.q, f);
+    const f32x2 c = fma2(p.q, mul2(p.y, pk1(-0.5f)), pk1(0.5f));
+    const f32x2 y = fma2(p.y, c, p.y);
+    const f32x2 r = fma2(p.q, c, p.q);
     const f32x2 v = mul2(y, y);
     const f32x2 v3 = mul2(mul2(v, v), v);
     const f32x2 ndisp = mul2(v3, fma2(v, fma2(v, E.nk10, E.nk8), E.nk6));   // -disp

@@ -229,7 +229,8 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
                 const double T_PB = -Dku * (lam + g2);
                 const double T_JF = -0.5 * Dku * lam;
                 double *o = out + (size_t)w * 4;
-                o[0] = c + T_PB; o[1] = c; o[2] = T_PB; o[3] = T_JF;
+                const double V = c * g.az.f32_scale;                                     // the potential was summed in units of f32_scale K
+                o[0] = V + T_PB; o[1] = V; o[2] = T_PB; o[3] = T_JF;
             }
         }
     }

@@ -279,7 +279,7 @@ def test_local_energy_fp64(qmc, oracle, N):
 
 
 @pytest.mark.parametrize("variant", [2, 0, 3])
-@pytest.mark.parametrize("N", [64, 256, 515, 1000, 1952])         # 515, 1000: ragged last block; odd and even block counts
+@pytest.mark.parametrize("N", [64, 100, 256, 515, 1000, 1952])    # 100, 515, 1000: ragged last block; odd and even block counts
 def test_local_energy_fp32c(qmc, oracle, tuning, N, variant):
     """fp32 coordinates + fp32 pair arithmetic vs the fp64 oracle on the SAME (fp32-exact) coordinates.
     The cutoff guard (R2): a pair within fp32 rounding of L/2 may be classified differently; V jumps
