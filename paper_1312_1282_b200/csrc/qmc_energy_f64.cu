@@ -91,7 +91,7 @@ struct Pending64 {
 struct Pair64 { double mx, my, mz, t, gm, lt, v, x, q, disp; bool in; };   // v = -dispersion sum: F = 1, no repulsive term (Pending64)
 
 // all terms of one pair; bias > 0 pushes the pair beyond the cutoff
-template <bool kEnergy, bool kPend>
+template <bool kEnergy, int kPend>
 __device__ __forceinline__ Pair64 pair64(double xi, double yi, double zi, double xs, double ys, double zs,
                                          double bias, const Const64 &C)
 {
@@ -118,7 +118,7 @@ __device__ __forceinline__ Pair64 pair64(double xi, double yi, double zi, double
         const double x = r * C.inv_rm;
         const double w = C.rm2 * y2;                                // 1/x^2
         const double disp = w * w * w * fma(w, fma(w, C.c10, C.c8), C.c6);
-        if (kPend) {
+        if (kPend != 0) {
             p.x = x;
             p.q = fma(C.Drm, y, -1.0);                              // D/x - 1
             p.disp = disp;
@@ -161,7 +161,51 @@ __device__ __forceinline__ void pending_park(Pending64 &Q, const Pair64 &p, cons
     if (hit) { Q.x = p.x; Q.q = p.q; Q.disp = p.disp; Q.full = true; }
 }
 
-template <int T, bool kEnergy, bool kPend>
+// kPend = 2, boxes small enough that a lane's pending slot would be evaluated almost every step (N = 512: 12.5 % of
+// the pairs have x < 3) and with room in shared memory: the warp COMPACTS such pairs into a queue of (x, dispersion)
+// and evaluates the exponentials 32 entries at a time, one per lane, so that their cost is paid once per near pair
+// instead of once per warp step.  The queue holds at most 31 + 64 entries.
+constexpr int kQueue64 = 96;
+struct Queue64 {
+    double *x, *d;
+    int cnt = 0;
+    double rep = 0.0, corr = 0.0;                    // sum of exp(..); sum of (1 - F) disp
+};
+__device__ __forceinline__ void queue_drain(Queue64 &Q, const Const64 &C, int first, int n, int lane)
+{
+    __syncwarp();
+    const bool act = lane < n;
+    const double x = act ? Q.x[first + lane] : 3.0;
+    const double e = exp_neg(x * fma(C.beta, x, -C.alpha));
+    Q.rep += act ? e : 0.0;
+    const bool damped = act && x < C.D;
+    if (__any_sync(0xffffffffu, damped)) {
+        const double d = act ? Q.d[first + lane] : 0.0;
+        double z;                                    // 1/x to third order
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(z) : "d"(x));
+        const double e1 = fma(-x, z, 1.0);
+        z = fma(z, fma(e1, e1, e1), z);
+        const double q = fma(C.D, z, -1.0);          // D/x - 1
+        const double F = exp_neg(-q * q);
+        Q.corr += damped ? (1.0 - F) * d : 0.0;
+    }
+    __syncwarp();
+}
+__device__ __forceinline__ void queue_push(Queue64 &Q, const Pair64 &p, int lane)
+{
+    const bool hit = p.in && __double2hiint(p.x) < kRepHi;
+    const unsigned m = __ballot_sync(0xffffffffu, hit);
+    if (m != 0u) {
+        if (hit) {
+            const int pos = Q.cnt + __popc(m & ((1u << lane) - 1u));
+            Q.x[pos] = p.x;
+            Q.d[pos] = p.disp;
+        }
+        Q.cnt += __popc(m);
+    }
+}
+
+template <int T, bool kEnergy, int kPend>
 __global__ void __launch_bounds__(T, (T <= 128 ? 4 : (T <= 256 ? 2 : 1)))
 energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
 {
@@ -202,6 +246,8 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
     const bool even = (nblk & 1) == 0;
     double tLam = 0.0, tV = 0.0;
     Pending64 Q;
+    Queue64 W;
+    if (kPend == 2) { W.x = ag + 4 * NP + warp * (2 * kQueue64); W.d = W.x + kQueue64; }
     double own[kMaxOwn64][4];                                         // G_x, G_y, G_z, S of this lane's particle in each own block
 #pragma unroll 1
     for (int a = 0; a < kMaxOwn64; ++a) { own[a][0] = 0.0; own[a][1] = 0.0; own[a][2] = 0.0; own[a][3] = 0.0; }
@@ -222,7 +268,7 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
             const bool vj = jb + lane < N;
             double gxj = 0.0, gyj = 0.0, gzj = 0.0, sj = 0.0;
             const int s0 = (k == 0) ? 1 : 0, s1 = (k == 0) ? 17 : 32;
-            if (kPend) {
+            if (kPend != 0) {
 #pragma unroll 1
                 for (int s = s0; s < s1; s += 2) {                        // two pairs per lane in flight (s1 - s0 is even)
                     const int srcA = (lane + s) & 31, srcB = (lane + s + 1) & 31;
@@ -245,7 +291,12 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
                         tV += pA.v; tV += pB.v;
                         gxj -= shfl_from(ax, fromA); gyj -= shfl_from(ay, fromA); gzj -= shfl_from(az, fromA);
                         gxj -= shfl_from(bx, fromB); gyj -= shfl_from(by, fromB); gzj -= shfl_from(bz, fromB);
-                        if (kPend) { pending_park(Q, pA, C); pending_park(Q, pB, C); }
+                        if (kPend == 1) { pending_park(Q, pA, C); pending_park(Q, pB, C); }
+                        if (kPend == 2) {
+                            queue_push(W, pA, lane);
+                            queue_push(W, pB, lane);
+                            while (W.cnt >= 32) { W.cnt -= 32; queue_drain(W, C, W.cnt, 32, lane); }
+                        }
                     }
                 }
             } else {
@@ -253,7 +304,7 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
                 for (int s = s0; s < s1; ++s) {                       // one pair per lane and step
                     const int src = (lane + s) & 31;
                     const bool ok = vi && (jb + src < N) && !(k == 0 && s == 16 && lane >= 16);
-                    const Pair64 p = pair64<kEnergy, false>(xi, yi, zi, x[jb + src], y[jb + src], z[jb + src], ok ? 0.0 : kBig, C);
+                    const Pair64 p = pair64<kEnergy, 0>(xi, yi, zi, x[jb + src], y[jb + src], z[jb + src], ok ? 0.0 : kBig, C);
                     si += p.t;
                     double cx = 0.0, cy = 0.0, cz = 0.0;
                     if (kEnergy) {
@@ -306,7 +357,8 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
         }
     }
     if (kEnergy) {
-        if (kPend) { pending_flush(Q, C); tV = fma(C.A, Q.rep, tV) + Q.corr; }
+        if (kPend == 1) { pending_flush(Q, C); tV = fma(C.A, Q.rep, tV) + Q.corr; }
+        if (kPend == 2) { queue_drain(W, C, 0, W.cnt, lane); tV = fma(C.A, W.rep, tV) + W.corr; }
         tV *= C.eps;
         // each unordered pair was seen once: the Laplacian sum over i counts it twice
         tLam *= 2.0;
@@ -333,7 +385,7 @@ energy64_kernel(StateView sv, double Dk, double *__restrict__ out)
 
 int smem_bytes64(int N) { return 98 * 8 + 7 * (((N + 31) >> 5) << 5) * 8; }
 
-template <int T, bool kEnergy, bool kPend>
+template <int T, bool kEnergy, int kPend>
 cudaError_t launch64k(qmc_ctx *c, double *d_out, int smem)
 {
     auto k = energy64_kernel<T, kEnergy, kPend>;
@@ -343,29 +395,35 @@ cudaError_t launch64k(qmc_ctx *c, double *d_out, int smem)
     return cudaGetLastError();
 }
 
-// The pending-slot form of the exponentials (Pending64) pays while few pairs are near: it is used when the sphere
-// x < 3 holds less than 5 % of the particles (N = 1952 at liquid density: 3.3 %; N = 512: 12.5 %).
-bool few_near_pairs(const qmc_ctx *c)
+// fraction of the particles inside the sphere x < 3 around a particle (the pairs that need the exponentials)
+double near_pair_fraction(const qmc_ctx *c)
 {
     double Lmin = c->box_L[0];
     for (double L : c->box_L) Lmin = L < Lmin ? L : Lmin;
     const double r = 3.0 * c->p.aziz[1];                 // r_m, Angstrom like box_L
-    return 4.18879 * r * r * r < 0.05 * Lmin * Lmin * Lmin;
+    return 4.18879 * r * r * r / (Lmin * Lmin * Lmin);
 }
 
+// How the exponentials are evaluated: 1 (per-lane pending slot) while few pairs are near (N = 1952 at liquid density:
+// 3.3 %); 2 (warp queue) for smaller boxes if two CTAs with their queues still fit an SM (N = 512: 12.5 %, N = 256:
+// 25 %); 0 (in place) when most pairs are near anyway (N = 64).
 template <int T>
 cudaError_t launch64(qmc_ctx *c, double *d_out, bool energy)
 {
     const int smem = smem_bytes64(c->p.N);
-    if (!energy) return launch64k<T, false, false>(c, d_out, smem);
-    return few_near_pairs(c) ? launch64k<T, true, true>(c, d_out, smem) : launch64k<T, true, false>(c, d_out, smem);
+    if (!energy) return launch64k<T, false, 0>(c, d_out, smem);
+    const double f = near_pair_fraction(c);
+    const int qbytes = (T >> 5) * 2 * kQueue64 * 8;
+    if (f < 0.05) return launch64k<T, true, 1>(c, d_out, smem);
+    if (f < 0.5 && 2 * (smem + qbytes + 1024) <= 228 * 1024) return launch64k<T, true, 2>(c, d_out, smem + qbytes);
+    return launch64k<T, true, 0>(c, d_out, smem);
 }
 
 template <int T>
 int occupancy64(int smem)
 {
     int occ = 0;
-    auto k = energy64_kernel<T, true, true>;
+    auto k = energy64_kernel<T, true, 1>;
     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, T, smem);
     return occ;
@@ -384,7 +442,7 @@ cudaError_t launch_energy_f64(qmc_ctx *c, double *d_out, bool energy)
     return cudaErrorInvalidValue;
 }
 
-// One warp per 64 particles (a block of 32 has about n/2 block pairs to go through), 1 to 8 warps;
+// 1 to 8 warps;
 // qmc_set_tuning("energy_threads") overrides (tuning experiments).  false: N too large for the per-particle
 // accumulators in shared memory -- the caller falls back to the ordered-pair kernel of qmc_energy.cu.
 bool plan_energy_f64(qmc_ctx *c, EnergyPlan *out)
@@ -392,8 +450,8 @@ bool plan_energy_f64(qmc_ctx *c, EnergyPlan *out)
     const int N = c->p.N;
     const int smem = smem_bytes64(N);
     if (smem > 227 * 1024) return false;
-    int T = 32;
-    while (2 * T < N && T < 256) T *= 2;
+    // measured (c2, c5, c3): 128 threads up to N ~ 1000 (N = 512: 13.6 ms against 13.9 with 256), 256 above
+    int T = N <= 64 ? 32 : (N <= 128 ? 64 : (N <= 1024 ? 128 : 256));
     if (g_tuning.energy_threads > 0) {
         const int v = g_tuning.energy_threads;
         if (v >= 32 && v <= 512 && ((v & (v - 1)) == 0 || v == 384)) T = v;
