@@ -33,8 +33,8 @@ from paper_1312_1282_b200 import workloads as wl  # noqa: E402
 ALG_INSTR = {wl.MODE_FP32C: 24.0, wl.MODE_FP64: 31.0}
 LANES_PER_SM = {wl.MODE_FP32C: 128, wl.MODE_FP64: 64}
 # DRAM bytes per launch of the dominant kernel from the ncu --set full capture of the same command
-# (profiles/r02_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum); None where no capture exists.
-NCU_TRAFFIC_BYTES = {("c3-N1952", wl.MODE_FP32C): 80.1e6 + 22.1e6, ("c3-N1952-fp64", wl.MODE_FP64): 129.7e6 + 69.4e6}
+# (profiles/r02b_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum); None where no capture exists.
+NCU_TRAFFIC_BYTES = {("c3-N1952", wl.MODE_FP32C): 80.0e6 + 22.4e6, ("c3-N1952-fp64", wl.MODE_FP64): 129.7e6 + 70.4e6}
 EQUIL_SWEEPS = {1: 200, 2: 200, 3: 150, 4: 20, 5: 60}      # untimed, before the warm-up (time the liquid, not the melting lattice)
 
 
@@ -377,7 +377,7 @@ def main():
         "achieved": achieved / 1e9, "peak": peak_derived / 1e9, "unit": "G thread-instr/s",
         "frac": achieved / peak_derived, "traffic": traffic,
         "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum per launch, ncu --set full of this command "
-                        "(profiles/r02_kernels.md); the walker state is 80 MB (fp32c) / 128 MB (fp64): read once, "
+                        "(profiles/r02b_kernels.md); the walker state is 80 MB (fp32c) / 128 MB (fp64): read once, "
                         "coordinates + S written once",
         "peak_source": f"derived: {info['sm_count']} SMs x {LANES_PER_SM[w.mode]} lanes x {sm_max:.0f} MHz (DESIGN.md); "
                        "MEASURED_PEAKS.json has no ALU entry",
