@@ -29,8 +29,9 @@ using namespace e32;
 // fixed-point grids of the per-particle accumulators: 2^-24 of a pair-sum term (t/32) and of a gradient term
 // (gm/128 times the minimum image in box units; the terms arrive times 2^32)
 constexpr double kFixS = 0x1p24, kFixG = 0x1p-8;
-__device__ __forceinline__ long long fix_s(float v) { return __float2ll_rn(v * 0x1p24f); }
-__device__ __forceinline__ long long fix_g(float v) { return __float2ll_rn(v * 0x1p-8f); }
+// bad: a partial sum that is not finite (two particles on one grid point) cannot be carried by a fixed-point number
+__device__ __forceinline__ long long fix_s(float v, bool &bad) { bad |= !(fabsf(v) <= 3.0e38f); return __float2ll_rn(v * 0x1p24f); }
+__device__ __forceinline__ long long fix_g(float v, bool &bad) { bad |= !(fabsf(v) <= 3.0e38f); return __float2ll_rn(v * 0x1p-8f); }
 // A 64-bit fixed-point accumulator is two 32-bit words, hi (signed, units of 2^24) and lo (unsigned): v = hi 2^24 +
 // lo with 0 <= lo < 2^24 is added by TWO native 32-bit shared-memory atomics (a 64-bit atomic add on shared memory is
 // a compare-and-swap loop).  A particle receives at most nblk + 1 <= 81 additions, so lo stays below 2^31 and no
@@ -158,6 +159,7 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
     const bool even = (nblk & 1) == 0, ragged = (N & 31) != 0;
     double tLam = 0.0, tLg = 0.0, tV = 0.0;
     f32x2 n_out2 = pk1(0.0f);                                         // clamped slots, per packed lane
+    bool bad = false;
     int k = warp / nblk, A = warp - k * nblk;                         // task t = warp, warp + nwarps, ...: k = t / n, A = t mod n
 #pragma unroll 1
     for (;;) {
@@ -182,29 +184,31 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
             tV += (double)hsum2(P.v);
         }
         if (jb + lane < N) {
-            fix_add(ag, 3 * NP + jb + lane, fix_s(hsum2(P.sj)));
+            fix_add(ag, 3 * NP + jb + lane, fix_s(hsum2(P.sj), bad));
             if (kEnergy) {
-                fix_add(ag, jb + lane, -fix_g(hsum2(P.gxj)));         // d_ji = -d_ij
-                fix_add(ag, NP + jb + lane, -fix_g(hsum2(P.gyj)));
-                fix_add(ag, 2 * NP + jb + lane, -fix_g(hsum2(P.gzj)));
+                fix_add(ag, jb + lane, -fix_g(hsum2(P.gxj), bad));         // d_ji = -d_ij
+                fix_add(ag, NP + jb + lane, -fix_g(hsum2(P.gyj), bad));
+                fix_add(ag, 2 * NP + jb + lane, -fix_g(hsum2(P.gzj), bad));
             }
         }
         if (vi) {
-            fix_add(ag, 3 * NP + i, fix_s(hsum2(P.si)));
+            fix_add(ag, 3 * NP + i, fix_s(hsum2(P.si), bad));
             if (kEnergy) {
-                fix_add(ag, i, fix_g(hsum2(P.gxi)));
-                fix_add(ag, NP + i, fix_g(hsum2(P.gyi)));
-                fix_add(ag, 2 * NP + i, fix_g(hsum2(P.gzi)));
+                fix_add(ag, i, fix_g(hsum2(P.gxi), bad));
+                fix_add(ag, NP + i, fix_g(hsum2(P.gyi), bad));
+                fix_add(ag, 2 * NP + i, fix_g(hsum2(P.gzi), bad));
             }
         }
         A += nwarps;
         while (A >= nblk) { A -= nblk; ++k; }
     }
-    __syncthreads();
+    // a singular configuration: the pair sums come out as NaN, as they would from a floating-point accumulator (the
+    // energies below are not finite then anyway: the Laplacian and potential totals are floating point)
+    const double poison = __syncthreads_or(bad) ? __longlong_as_double(0x7ff8000000000000LL) : 0.0;
 
     double tG2 = 0.0;
     for (int i = tid; i < N; i += T) {
-        sv.S[(size_t)w * ld + i] = fix_get(ag, 3 * NP + i) * (kSUnit / kFixS);     // R17: rebuild the running sum
+        sv.S[(size_t)w * ld + i] = fix_get(ag, 3 * NP + i) * (kSUnit / kFixS) + poison;     // R17: rebuild the running sum
         if (kEnergy) {
             const double a = fix_get(ag, i) * (1.0 / kFixG), b = fix_get(ag, NP + i) * (1.0 / kFixG), c = fix_get(ag, 2 * NP + i) * (1.0 / kFixG);
             tG2 += a * a + b * b + c * c;

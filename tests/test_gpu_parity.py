@@ -327,6 +327,24 @@ def test_local_energy_reproducible_to_the_bit(qmc, mode_name, N):
     assert torch.equal(q2.pair_sums(), S0[20:27])
 
 
+def test_local_energy_fp32c_singular_configuration_is_not_finite(qmc):
+    """Two particles on one grid point: the pair sums of that walker come out as NaN and its energies are not
+    finite (the fixed-point accumulators of the unordered-pair kernel cannot carry an infinity by themselves); the
+    other walkers of the launch are untouched."""
+    N, W = 256, 3
+    q, L = make(qmc, N, W, qmc.QMC_FP32C)
+    xyz = np.stack([wl.liquid_configuration(N, L, 310 + k, fp32_grid=True) for k in range(W)])
+    good = xyz.copy()
+    xyz[1, :, 17] = xyz[1, :, 200]
+    q.set_positions(good)
+    e_good, S_good = q.local_energy().cpu().numpy(), q.pair_sums().cpu().numpy()
+    q.set_positions(xyz)
+    e, S = q.local_energy().cpu().numpy(), q.pair_sums().cpu().numpy()
+    assert not np.isfinite(e[1]).any() or not np.isfinite(e[1, 0])
+    assert np.isnan(S[1]).all()
+    assert np.array_equal(e[[0, 2]], e_good[[0, 2]]) and np.array_equal(S[[0, 2]], S_good[[0, 2]])
+
+
 @pytest.mark.parametrize("N,W", [(64, 16), (256, 4)])
 def test_local_energy_fp32c_equilibrated_liquid(qmc, oracle, N, W):
     """The regime the tolerance is hardest in: an EQUILIBRATED liquid (E = V + T cancels ~3.5x).  The
