@@ -19,7 +19,8 @@
 //
 // Cutoff: r^2 is clamped to h^2 for the arithmetic (nothing overflows) and the four pair terms of a pair
 // beyond the cutoff, of a padding slot, or of the inactive half of the last diagonal step are selected to
-// exactly 0 -- one DSETP on the fp64 pipe, the selects run on the integer pipe.
+// exactly 0 -- comparison (on the bit patterns, less_pos) and selects on the integer pipe.
+// The two exponentials of HFD-B(HE) are kept out of the pair loop where that pays (kPend, below).
 #include "qmc_internal.h"
 
 namespace qmc {

@@ -16,8 +16,9 @@
 // FILTERED evaluation (round 2; the bits above are unchanged).  The specified arithmetic costs ~30 fp64 instructions
 // per pair, among them a correctly rounded square root.  The kernel first computes the bin coordinate u = r nbins / h
 // in fp32 from 32-bit fixed-point coordinates (the FP32C representation of qmc_f32c.cuh; in FP64 mode the coordinates
-// rounded to 2^-32 of the box; the fp64 coordinates stay in global memory): wrapping integer differences, r^2, r = r^2 rsqrt(r^2), u.  Its error against the
-// specified fp64 value is below 2e-6 u (rsqrt.approx 2^-22, four fp32 roundings, coordinate rounding 2^-33 L), i.e.
+// rounded to 2^-32 of the box; the fp64 coordinates stay in global memory): wrapping integer differences, r^2,
+// r = sqrt.approx(r^2), u.  Its error against the specified fp64 value is below 2e-6 u (sqrt.approx 2^-22, four fp32
+// roundings, coordinate rounding 2^-33 L), i.e.
 // below 1e-3 of a bin for nbins <= 512 (4e-4 with the roundings of the floor itself).  If floor(u - kGuard) == floor(u + kGuard) the pair is that far from every bin
 // edge and from the cutoff (u = nbins), so the specified arithmetic gives the same bin: it is counted at once.
 // Otherwise (2 kGuard = 0.4 % of the pairs) the pair goes to a per-warp queue that evaluates the specified fp64
