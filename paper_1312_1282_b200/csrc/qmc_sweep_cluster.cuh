@@ -170,6 +170,8 @@ sweep_cluster_kernel(StateView sv, TraceView tr, uint2 key, uint32_t t0, int n_s
 
     unsigned long long n_acc = 0;
     int s = 0;
+    constexpr int kMoveUnroll = kF32 ? 4 : 1;                 // as in the one-block kernel (qmc_sweep_impl.cuh)
+#pragma unroll kMoveUnroll
     for (uint32_t m = 0; m < total; ++m) {
         if ((m & (kChunk - 1)) == 0) produce((m >> 5) + 1, (int)(((m >> 5) + 1) & 1));
         const MoveRand<Real> mr = fetch(m);
