@@ -57,13 +57,13 @@ struct SymAcc {            // fp32 partial sums of up to 16 packed steps
 // npk packed steps (2 npk pairs) of one block pair, starting at step s0 (step s pairs lane l with j-lane (l+s) & 31):
 // npk = 16, s0 = 0 for a full block pair, npk = 8, s0 = 1 for the diagonal block.
 //   kBias: some slots must be forced beyond the cutoff (padding particles, second half of diagonal step 16)
-template <bool kEnergy, bool kBias>
+template <bool kEnergy, bool kBias, int kUnroll>
 __device__ __forceinline__ void sym_steps(const int4 *__restrict__ xyz,
                                             int jb, int s0, int npk, int lane, bool vi, int N, bool diag,
                                             int32_t xi, int32_t yi, int32_t zi, const AzizF32 &E, int32_t zero,
                                             SymAcc &P, f32x2 &n_out2)
 {
-#pragma unroll 4
+#pragma unroll kUnroll
     for (int p = 0; p < npk; ++p) {
         const int sa = s0 + 2 * p, sb = sa + 1;
         const int ja = (lane + sa) & 31, jl = (lane + sb) & 31;
@@ -115,6 +115,9 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
     const int N = sv.N, ld = sv.ld;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int nwarps = T >> 5;
+    // packed pair steps in flight per lane: 4 with 128 registers (T <= 256, T = 512), 2 with the 85 of T = 384
+    // (measured: 10.01 against 10.34 ms with 2 at T = 256; 9.05 against 9.12 ms with 4 at T = 384)
+    constexpr int kSteps = (T == 384) ? 2 : 4;
     const int w = blockIdx.x;
     const int nblk = (N + 31) >> 5, NP = nblk << 5;
 
@@ -176,8 +179,8 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
         SymAcc P;
         P.gxi = P.gyi = P.gzi = P.si = P.gxj = P.gyj = P.gzj = P.sj = P.lam = P.lg = P.v = pk1(0.0f);
         const int s0 = diag ? 1 : 0, npk = diag ? 8 : 16;
-        if (bias) sym_steps<kEnergy, true>(xyz, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_out2);
-        else      sym_steps<kEnergy, false>(xyz, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_out2);
+        if (bias) sym_steps<kEnergy, true, kSteps>(xyz, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_out2);
+        else      sym_steps<kEnergy, false, kSteps>(xyz, jb, s0, npk, lane, vi, N, diag, xi, yi, zi, E, zero, P, n_out2);
         if (kEnergy) {
             tLam += (double)hsum2(P.lam);
             tLg += (double)hsum2(P.lg);
@@ -291,6 +294,7 @@ bool plan_energy_f32s(qmc_ctx *c, EnergyPlan *out)
     if (smem > 113 * 1024) return false;
     int T = 32;
     while (2 * T < N && T < 256) T *= 2;
+    if (N >= 1536) T = 384;              // 24 warps per SM at 80 registers beat 16 at 128 (9.32 -> 9.12 ms at N = 1952)
     if (g_tuning.energy_threads > 0) {
         const int v = g_tuning.energy_threads;
         if (v >= 32 && v <= 512 && ((v & (v - 1)) == 0 || v == 384)) T = v;
