@@ -87,28 +87,37 @@ struct HistCtx {
     int in_limit;
 };
 
-// one pair per lane (same j for all lanes); kMask: some lanes hold no valid pair.  Counts the pair if it is clear of
-// every bin edge, else returns true: the pair needs the specified arithmetic.
-template <bool kFilter, bool kMask>
-__device__ __forceinline__ bool hist_pair(const HistCtx &C, int32_t xi, int32_t yi, int32_t zi, int32_t X, int32_t Y, int32_t Z, bool valid)
+// Two pairs per lane (particles j, j + 1: the same two j for all lanes) in packed fp32; kMask: some lanes hold no
+// valid pair.  A pair that is clear of every bin edge and of the cutoff is counted at once (predicated shared-memory
+// reduction: a branch around atomicAdd costs BSSY / BRA / BSYNC per pair; Hs = shared-window address of bin 0 minus
+// 4 x 0x4B000000); slow = true: the pair needs the specified arithmetic.  sqrt(0) = 0 lands in the guard band of bin 0.
+template <bool kMask>
+__device__ __forceinline__ void hist_pair2(const HistCtx &C, int32_t xi, int32_t yi, int32_t zi, int32_t X0, int32_t X1,
+                                           int32_t Y0, int32_t Y1, int32_t Z0, int32_t Z1, bool valid0, bool valid1,
+                                           bool &slow0, bool &slow1)
 {
-    if (!kFilter) return kMask ? valid : true;
-    const float mx = __int2float_rn(wsub(xi, X));
-    const float my = __int2float_rn(wsub(yi, Y));
-    const float mz = __int2float_rn(wsub(zi, Z));
-    const float r2 = fmaf(mx, mx, fmaf(my, my, mz * mz));
-    float rr;                                                         // r / L times 2^32; sqrt(0) = 0 lands in the guard band of bin 0
-    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(rr) : "f"(r2));
-    const int b0 = __float_as_int(fmaf(rr, C.uscale, C.lo_off) + 8388608.0f);         // 2^23 + floor(u - guard)
-    const int b1 = __float_as_int(fmaf(rr, C.uscale, C.hi_off) + 8388608.0f);         // 2^23 + floor(u + guard)
-    bool slow = b0 != b1;                                             // near a bin edge or the cutoff
-    if (kMask) slow = slow && valid;
-    const bool count = kMask ? (valid && !slow && b1 < C.in_limit) : (!slow && b1 < C.in_limit);
-    // predicated reduction instead of a branch around atomicAdd (the branch costs BSSY / BRA / BSYNC per pair);
-    // Hs = shared-window address of bin 0 minus 4 x 0x4B000000
+    const f32x2 mx = pk2(__int2float_rn(wsub(xi, X0)), __int2float_rn(wsub(xi, X1)));
+    const f32x2 my = pk2(__int2float_rn(wsub(yi, Y0)), __int2float_rn(wsub(yi, Y1)));
+    const f32x2 mz = pk2(__int2float_rn(wsub(zi, Z0)), __int2float_rn(wsub(zi, Z1)));
+    const f32x2 r2 = fma2(mx, mx, fma2(my, my, mul2(mz, mz)));
+    float ra, rb;
+    upk2(r2, ra, rb);
+    asm("sqrt.approx.ftz.f32 %0, %0;" : "+f"(ra));
+    asm("sqrt.approx.ftz.f32 %0, %0;" : "+f"(rb));
+    const f32x2 rr = pk2(ra, rb), us = pk1(C.uscale), magic = pk1(8388608.0f);
+    float l0, l1, h0, h1;
+    upk2(add2(fma2(rr, us, pk1(C.lo_off)), magic), l0, l1);           // 2^23 + floor(u - guard), both pairs
+    upk2(add2(fma2(rr, us, pk1(C.hi_off)), magic), h0, h1);           // 2^23 + floor(u + guard)
+    const int a0 = __float_as_int(l0), a1 = __float_as_int(l1), b0 = __float_as_int(h0), b1 = __float_as_int(h1);
+    slow0 = a0 != b0;
+    slow1 = a1 != b1;
+    if (kMask) { slow0 = slow0 && valid0; slow1 = slow1 && valid1; }
+    const bool c0 = kMask ? (valid0 && !slow0 && b0 < C.in_limit) : (!slow0 && b0 < C.in_limit);
+    const bool c1 = kMask ? (valid1 && !slow1 && b1 < C.in_limit) : (!slow1 && b1 < C.in_limit);
     asm volatile("{ .reg .pred p; setp.ne.s32 p, %2, 0; @p red.shared.add.u32 [%0], %1; }"
-                 :: "r"(C.Hs + 4u * (uint32_t)b1), "r"(1u), "r"((int)count) : "memory");
-    return slow;
+                 :: "r"(C.Hs + 4u * (uint32_t)b0), "r"(1u), "r"((int)c0) : "memory");
+    asm volatile("{ .reg .pred p; setp.ne.s32 p, %2, 0; @p red.shared.add.u32 [%0], %1; }"
+                 :: "r"(C.Hs + 4u * (uint32_t)b1), "r"(1u), "r"((int)c1) : "memory");
 }
 __device__ __forceinline__ void hist_enqueue(HistCtx &C, bool slow, int i, int j, int lane)
 {
@@ -191,17 +200,21 @@ __global__ void __launch_bounds__(256, 4) pair_histogram_kernel(StateView sv, in
             const int4 Z = *reinterpret_cast<const int4 *>(fz + jb + jj);
             const int j = jb + jj;
             bool s0, s1, s2, s3;
-            if (masked) {
+            if (!kFilter) {
                 const bool vi = i < N;
-                s0 = hist_pair<kFilter, true>(C, xi, yi, zi, X.x, Y.x, Z.x, vi && j < N && (k != 0 || j > i));
-                s1 = hist_pair<kFilter, true>(C, xi, yi, zi, X.y, Y.y, Z.y, vi && j + 1 < N && (k != 0 || j + 1 > i));
-                s2 = hist_pair<kFilter, true>(C, xi, yi, zi, X.z, Y.z, Z.z, vi && j + 2 < N && (k != 0 || j + 2 > i));
-                s3 = hist_pair<kFilter, true>(C, xi, yi, zi, X.w, Y.w, Z.w, vi && j + 3 < N && (k != 0 || j + 3 > i));
+                s0 = vi && j < N && (k != 0 || j > i);
+                s1 = vi && j + 1 < N && (k != 0 || j + 1 > i);
+                s2 = vi && j + 2 < N && (k != 0 || j + 2 > i);
+                s3 = vi && j + 3 < N && (k != 0 || j + 3 > i);
+            } else if (masked) {
+                const bool vi = i < N;
+                hist_pair2<true>(C, xi, yi, zi, X.x, X.y, Y.x, Y.y, Z.x, Z.y, vi && j < N && (k != 0 || j > i),
+                                 vi && j + 1 < N && (k != 0 || j + 1 > i), s0, s1);
+                hist_pair2<true>(C, xi, yi, zi, X.z, X.w, Y.z, Y.w, Z.z, Z.w, vi && j + 2 < N && (k != 0 || j + 2 > i),
+                                 vi && j + 3 < N && (k != 0 || j + 3 > i), s2, s3);
             } else {
-                s0 = hist_pair<kFilter, false>(C, xi, yi, zi, X.x, Y.x, Z.x, true);
-                s1 = hist_pair<kFilter, false>(C, xi, yi, zi, X.y, Y.y, Z.y, true);
-                s2 = hist_pair<kFilter, false>(C, xi, yi, zi, X.z, Y.z, Z.z, true);
-                s3 = hist_pair<kFilter, false>(C, xi, yi, zi, X.w, Y.w, Z.w, true);
+                hist_pair2<false>(C, xi, yi, zi, X.x, X.y, Y.x, Y.y, Z.x, Z.y, true, true, s0, s1);
+                hist_pair2<false>(C, xi, yi, zi, X.z, X.w, Y.z, Y.w, Z.z, Z.w, true, true, s2, s3);
             }
             if (__any_sync(0xffffffffu, s0 || s1 || s2 || s3)) {     // one vote per four pairs on the common path
                 hist_enqueue(C, s0, i, j, lane);
