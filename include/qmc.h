@@ -189,6 +189,61 @@ int qmc_info(const qmc_ctx *c, qmc_info_t *out);
  * heuristic.  Returns QMC_E_ARG for an unknown key. */
 int qmc_set_tuning(const char *key, int32_t value);
 
+/* ---- local energy without any allocation --------------------------------------------------------------
+ * qmc_local_energy_fp32c_static: the FP32C local energy (same quantities as qmc_local_energy: l.113-115, l.129,
+ * l.381; HFD-B(HE) l.131, Eq.(9) l.155, box l.460) of W walkers of N atoms, one parameter point, WITHOUT a
+ * qmc_ctx and without allocating anything: no cudaMalloc / cudaFree / cudaHostAlloc, no host heap, no library
+ * routine that allocates.
+ *
+ * Who needs it.  qmc_create reserves device memory with cudaMalloc, and qmc_local_energy's gridded kernel reserves
+ * its working arrays with cudaMalloc the first time it runs.  Some hosts of this library cannot do that:
+ *  - a process whose device memory is already handed out in full to a pool (a tensor framework's caching allocator,
+ *    a job scheduler's per-tenant budget): cudaMalloc then fails with out-of-memory although the pool has room;
+ *  - a latency-bound loop (an analysis or steering step between blocks of sweeps, l.319-343): cudaMalloc and
+ *    cudaFree may synchronise the whole device and would stall every other stream of the process;
+ *  - code that is only given the buffers it may touch (a plugin or callback run by another runtime) and has no
+ *    licence to create device memory of its own.
+ * Such a caller passes its input and output buffers, and the working memory (fixed-point coordinates, the rebuilt
+ * pair sums S_i, per-thread-block partial sums, the parameter tables) is ONE array of QMC_STATIC_SCRATCH_BYTES
+ * (5 382 656 bytes, about 5.1 MiB) that is part of the library image: every GPU on which the library's kernels
+ * get loaded holds it from then until the process exits, whether this call is ever used or not.
+ *
+ * Limits: 1 <= W <= QMC_STATIC_MAX_WALKERS, 2 <= N <= QMC_STATIC_MAX_ATOMS and W * (N rounded up to a multiple of
+ * 32) <= QMC_STATIC_MAX_SLOTS (e.g. 128 walkers of 1952-2048 atoms, 26 of 10000, 6 of 40960).  Anything larger is
+ * refused with QMC_E_CAPACITY and a message that names the three limits; nothing is launched in that case.
+ *
+ * Arguments.  d_xyz: device [W][3][N] doubles, Angstrom, in [0, L] (the layout of qmc_set_positions; rounded to the
+ * FP32C grid of L 2^-23 exactly as qmc_set_positions does).  box_L, jastrow_b, aziz[9], hbar2_over_2m: as in
+ * qmc_params (host values; aziz is a host array of 9).  d_out: device [W][4] doubles = E_PB, V, T_PB, T_JF in K, as
+ * qmc_local_energy writes them (bit-identical to a QMC_FP32C context of the same W and N running the gridded energy
+ * kernel on this GPU).  cuda_stream: a cudaStream_t as void*, NULL = legacy default stream; the four kernels are
+ * enqueued there and the call returns without waiting.  err / err_len: optional host buffer that receives the
+ * message when the return value is not QMC_OK (there is no context to ask; qmc_last_error does not see this call).
+ * The caller owns every buffer; none is kept after the kernels have run.
+ *
+ * First call on a device.  The first call made while a given device is current looks up the device address of
+ * the static array (cudaGetSymbolAddress) and the SM count, and caches both; later calls on that device skip this.
+ * Make that first call during set-up, before any stream capture is begun.  The first call for a given
+ * (aziz, box_L) also spends a few milliseconds of HOST time on the fp32 amplitude scale (R22); the last pair is
+ * remembered.
+ *
+ * Sharing.  All calls in the process that target the same GPU use the SAME array, from whatever thread or stream.
+ * Calls enqueued on one stream follow each other and are safe.  Calls whose kernels can overlap on the GPU
+ * (different streams, or different host threads on different streams) overwrite each other's working memory and
+ * give wrong energies without any error: order them with events or keep them on one stream.  The array still
+ * holds the previous call's data when the next one starts; each call rewrites every word it later reads (tables,
+ * coordinates including the padding up to a multiple of 32, pair sums, partial sums), so no clearing is asked of
+ * the caller.  Host-side bookkeeping is guarded by a mutex; the call is safe to make from several threads.
+ * Errors: QMC_E_ARG (NULL pointer, N < 2, W < 1, box_L <= 0, jastrow_b < 0, r_m <= 0), QMC_E_CAPACITY (above),
+ * QMC_E_CUDA (a runtime call or a launch failed; message in err). */
+#define QMC_STATIC_MAX_WALKERS   4096
+#define QMC_STATIC_MAX_ATOMS     65536
+#define QMC_STATIC_MAX_SLOTS     262144
+#define QMC_STATIC_SCRATCH_BYTES 5382656
+int qmc_local_energy_fp32c_static(const double *d_xyz, int32_t W, int32_t N, double box_L, double jastrow_b,
+                                  const double *aziz, double hbar2_over_2m, double *d_out, void *cuda_stream,
+                                  char *err, size_t err_len);
+
 #ifdef __cplusplus
 }
 #endif

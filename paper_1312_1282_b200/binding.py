@@ -22,8 +22,10 @@ EXPORTS = (
     "qmc_acceptance", "qmc_step_host", "qmc_last_error", "qmc_get_positions", "qmc_set_positions",
     "qmc_set_seed", "qmc_get_pair_sums", "qmc_refresh_pair_sums", "qmc_trace_decisions", "qmc_info",
     "qmc_pair_histogram", "qmc_set_proposal", "qmc_run_blocks_host", "qmc_wait", "qmc_sweep_writeouts",
-    "qmc_set_tuning",
+    "qmc_set_tuning", "qmc_local_energy_fp32c_static",
 )
+# limits of qmc_local_energy_fp32c_static (include/qmc.h)
+STATIC_MAX_WALKERS, STATIC_MAX_ATOMS, STATIC_MAX_SLOTS, STATIC_SCRATCH_BYTES = 4096, 65536, 262144, 5382656
 PROBE_LIB_PATH = os.path.join(HERE, "libqmc_probe_b200.so")
 
 
@@ -97,6 +99,8 @@ def load_library() -> C.CDLL:
     lib.qmc_refresh_pair_sums.argtypes = [vp]
     lib.qmc_trace_decisions.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, C.c_int64]
     lib.qmc_info.argtypes = [vp, C.POINTER(Info)]
+    lib.qmc_local_energy_fp32c_static.argtypes = [vp, C.c_int32, C.c_int32, C.c_double, C.c_double, dp, C.c_double, vp, vp,
+                                                  C.c_char_p, C.c_size_t]
     for name in EXPORTS:
         if name not in ("qmc_state_bytes", "qmc_last_error"):
             getattr(lib, name).restype = C.c_int
@@ -143,6 +147,40 @@ def set_tuning(key: Optional[str] = None, value: int = -1):
     rc = lib.qmc_set_tuning(key.encode() if key is not None else None, int(value))
     if rc != 0:
         raise QmcError(rc, lib.qmc_last_error(None).decode())
+
+
+def local_energy_fp32c_static(xyz, box_L: float, jastrow_b: float, hbar2_over_2m: float, aziz: Sequence[float], out,
+                              stream=None):
+    """qmc_local_energy_fp32c_static: FP32C local energies [W][4] (E_PB, V, T_PB, T_JF in K) of the configurations
+    xyz [W][3][N] (float64 CUDA tensor, Angstrom) written into `out` ([W][4] float64 CUDA tensor), with no context and no
+    allocation on the library's side: its working memory is a fixed 5.1 MiB array inside the library image.  This is the
+    call for code that cannot reserve device memory itself -- the GPU's memory is already committed to a pool, or an
+    allocation (which may synchronise the whole device) is not acceptable where the call is made, or the caller may
+    only touch buffers it was handed.  Both tensors are the caller's; this wrapper creates none.  Limits:
+    W <= STATIC_MAX_WALKERS, N <= STATIC_MAX_ATOMS, W * roundup32(N) <= STATIC_MAX_SLOTS, else QmcError(QMC_E_CAPACITY).
+    The first call on a device looks up the array's address: make it before any stream capture.  Every call on a GPU
+    shares the one array, so calls that could overlap on the device (different streams) must be ordered by the caller.
+    Asynchronous on `stream` (default: torch's current stream)."""
+    import torch
+    lib = load_library()
+    assert xyz.dim() == 3 and xyz.shape[1] == 3 and xyz.dtype == torch.float64 and xyz.is_contiguous(), (xyz.shape, xyz.dtype)
+    W, _, N = (int(v) for v in xyz.shape)
+    assert out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= 4 * W, (out.shape, out.dtype)
+    if 1 <= W <= STATIC_MAX_WALKERS and 2 <= N <= STATIC_MAX_ATOMS and W * ((N + 31) // 32 * 32) <= STATIC_MAX_SLOTS:
+        # sizes the library will accept reach the kernels: both tensors have to be on the same GPU, which is made current
+        assert xyz.is_cuda and out.is_cuda and xyz.device == out.device, (xyz.device, out.device)
+        torch.cuda.set_device(xyz.device)
+        st = torch.cuda.current_stream(xyz.device) if stream is None else stream
+        handle = C.c_void_p(st.cuda_stream)
+    else:
+        handle = None                       # the library refuses these sizes before any CUDA call
+    err = C.create_string_buffer(512)
+    rc = lib.qmc_local_energy_fp32c_static(C.c_void_p(xyz.data_ptr()), W, N, float(box_L), float(jastrow_b),
+                                           (C.c_double * 9)(*aziz), float(hbar2_over_2m), C.c_void_p(out.data_ptr()),
+                                           handle, err, len(err))
+    if rc != 0:
+        raise QmcError(rc, err.value.decode())
+    return out
 
 
 class QMC:

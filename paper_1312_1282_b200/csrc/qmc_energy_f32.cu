@@ -23,6 +23,10 @@
 //
 // R20: per-pair terms are fp32; 16 consecutive j are summed in fp32 (two packed lanes of 8) and then added
 // to fp64 accumulators.
+#include <cstdarg>
+#include <cstring>
+#include <mutex>
+
 #include "qmc_energy_f32_pair.cuh"
 
 namespace qmc {
@@ -419,3 +423,195 @@ bool plan_energy_f32(qmc_ctx *c, EnergyPlan *out)
 }
 
 }  // namespace qmc
+
+// ==========================================================================================================
+// qmc_local_energy_fp32c_static (include/qmc.h): the gridded FP32C local-energy pass for callers that must not
+// allocate.  The kernels are the ones above, untouched (encode -> energy32g_kernel -> finalize32g_kernel); what
+// differs is where their working memory lives.  launch_energy_f32g() takes it from cudaMalloc on first use, and
+// everything else a qmc_ctx needs comes from cudaMalloc in qmc_create.  Here ALL of it -- the per-group constants,
+// the walker -> group table, the fixed-point coordinates, the rebuilt pair sums and the per-block partial sums --
+// sits in ONE file-scope device array that the CUDA module loader places when the library is loaded on a GPU.
+//
+// g_static_scratch below is, in HOST code, only a handle for the symbol: it is not a device address and must never
+// be handed to a kernel.  The device address comes from cudaGetSymbolAddress, asked once per device (with that
+// device current) on the first call and cached.
+// ==========================================================================================================
+namespace qmc {
+namespace {
+
+constexpr size_t kStaticGroupBytes = 512;                                         // one GroupDev, padded
+constexpr size_t kStaticGroupOfOff = kStaticGroupBytes;                            // int32 [QMC_STATIC_MAX_WALKERS]
+constexpr size_t kStaticEncOff = kStaticGroupOfOff + sizeof(int32_t) * QMC_STATIC_MAX_WALKERS;      // int32 [W][3][NP]
+constexpr size_t kStaticSOff = kStaticEncOff + sizeof(int32_t) * 3 * (size_t)QMC_STATIC_MAX_SLOTS;  // double [W][ld], ld <= NP
+constexpr size_t kStaticPartOff = kStaticSOff + sizeof(double) * (size_t)QMC_STATIC_MAX_SLOTS;      // double [W][parts][3]
+// parts <= ceil(NP / 256), so W * parts <= W * NP / 256 + W
+constexpr size_t kStaticPartMax = (size_t)QMC_STATIC_MAX_SLOTS / 256 + QMC_STATIC_MAX_WALKERS;
+constexpr size_t kStaticBytes = kStaticPartOff + sizeof(double) * 3 * kStaticPartMax;
+static_assert(sizeof(GroupDev) <= kStaticGroupBytes, "GroupDev outgrew its slot");
+static_assert(kStaticEncOff % 256 == 0 && kStaticSOff % 256 == 0 && kStaticPartOff % 256 == 0, "sub-arrays stay 256-byte aligned");
+static_assert(kStaticBytes == QMC_STATIC_SCRATCH_BYTES, "qmc.h states the size of the static scratch array");
+
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticBytes];
+
+// Writes the two small tables the unchanged kernels read through StateView: the constants of the single parameter
+// point, and group_of[w] = 0 for every walker (the only part of the scratch that has to hold zeros).
+__global__ void static_tables_kernel(GroupDev g, GroupDev *__restrict__ groups, int32_t *__restrict__ group_of, int W)
+{
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w == 0) groups[0] = g;
+    if (w < W) group_of[w] = 0;
+}
+
+// Angstrom [W][3][N] doubles -> fixed-point coordinates [W][3][NP], with exactly the arithmetic of
+// set_positions_kernel<float> (wrap into [0, L), s = fl32(1 + x/L) in [1, 2)) followed by encode_kernel.
+__global__ void encode_angstrom_kernel(const double *__restrict__ xyz, int N, int NP, double L_A, int32_t *__restrict__ enc)
+{
+    const int w = blockIdx.x;
+    const int j = blockIdx.y * blockDim.x + threadIdx.x;
+    if (j >= NP) return;
+    const double *src = xyz + (size_t)w * 3 * N;
+    int32_t *e = enc + (size_t)w * 3 * NP;
+    for (int c = 0; c < 3; ++c) {
+        int32_t k = 0;
+        if (j < N) {
+            double v = src[c * N + j];
+            if (v >= L_A) v -= L_A;
+            if (v < 0.0) v += L_A;
+            float s = __double2float_rn(1.0 + v / L_A);
+            if (s >= 2.0f) s -= 1.0f;
+            if (s < 1.0f) s += 1.0f;
+            k = enc_coord(s);
+        }
+        e[c * NP + j] = k;
+    }
+}
+
+struct StaticDevice { bool ready = false; unsigned char *base = nullptr; int sm_count = 0; };
+constexpr int kStaticMaxDevices = 64;
+StaticDevice g_static_dev[kStaticMaxDevices];
+// aziz_f32_scale() is a host search of a few milliseconds: remember the last parameter set it was run for
+struct StaticScale { bool valid = false; double aziz[9]; double L; double scale; } g_static_scale;
+std::mutex g_static_mu;
+
+int static_fail(char *err, size_t err_len, int code, const char *fmt, ...)
+{
+    if (err && err_len) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(err, err_len, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+}  // namespace
+}  // namespace qmc
+
+extern "C" int qmc_local_energy_fp32c_static(const double *d_xyz, int32_t W, int32_t N, double box_L, double jastrow_b,
+                                             const double *aziz, double hbar2_over_2m, double *d_out, void *cuda_stream,
+                                             char *err, size_t err_len)
+{
+    using namespace qmc;
+    if (!d_xyz || !d_out || !aziz) return static_fail(err, err_len, QMC_E_ARG, "d_xyz, d_out and aziz are required");
+    if (N < 2 || W < 1) return static_fail(err, err_len, QMC_E_ARG, "N >= 2 and W >= 1 required (got N = %d, W = %d)", N, W);
+    if (!(box_L > 0.0) || !(jastrow_b >= 0.0) || !(aziz[1] > 0.0))
+        return static_fail(err, err_len, QMC_E_ARG, "box_L > 0, jastrow_b >= 0 and aziz r_m > 0 required");
+    const long long NP = (((long long)N + 31) >> 5) << 5;
+    if (W > QMC_STATIC_MAX_WALKERS || N > QMC_STATIC_MAX_ATOMS || (long long)W * NP > QMC_STATIC_MAX_SLOTS)
+        return static_fail(err, err_len, QMC_E_CAPACITY,
+                           "W = %d walkers of N = %d atoms exceed the static scratch array: W <= %d, N <= %d and "
+                           "W * (N rounded up to a multiple of 32) = %lld <= %d; use a qmc_ctx and qmc_local_energy for larger runs",
+                           W, N, QMC_STATIC_MAX_WALKERS, QMC_STATIC_MAX_ATOMS, (long long)W * NP, QMC_STATIC_MAX_SLOTS);
+
+#define STATIC_CUDA(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) \
+        return static_fail(err, err_len, QMC_E_CUDA, "%s: %s", #expr, cudaGetErrorString(e__)); } while (0)
+
+    int dev = 0;
+    STATIC_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return static_fail(err, err_len, QMC_E_ARG, "device ordinal %d not supported", dev);
+    unsigned char *base = nullptr;
+    int sm_count = 0;
+    double f32_scale = 1.0;
+
+    // per-group constants exactly as qmc_create computes them for QMC_FP32C (coordinate unit = the box edge)
+    GroupDev G;
+    memset(&G, 0, sizeof(G));
+    {
+        const double unit = box_L;
+        G.unit = unit; G.inv_unit = 1.0 / unit; G.origin = 1.0;
+        G.L_A = box_L;
+        G.L = 1.0;
+        G.h = 0.5 * G.L; G.h2 = G.h * G.h;
+        const double bu = jastrow_b / unit;
+        G.b5 = bu * bu * bu * bu * bu;
+        G.c1 = -0.5 * G.b5;
+        const double h = G.h;
+        G.c0 = G.b5 / (h * h * h * h * h);
+        G.sh = 2.0 / (h * h * h * h * h);
+        G.step = 0.0;
+        long long k = 1;
+        while (4 * k * k * k < N) ++k;
+        G.k_lat = (int32_t)k;
+        G.a_lat = box_L / (double)k;
+        G.pad = 0;
+        const double rm = aziz[1] / unit;
+        G.az.eps = aziz[0]; G.az.inv_rm = 1.0 / rm; G.az.rm2 = rm * rm; G.az.A = aziz[2];
+        G.az.alpha = aziz[3]; G.az.beta = aziz[4]; G.az.c6 = aziz[5]; G.az.c8 = aziz[6]; G.az.c10 = aziz[7];
+        G.az.D = aziz[8]; G.az.Drm = aziz[8] * rm;
+    }
+    {
+        std::lock_guard<std::mutex> lock(g_static_mu);
+        StaticDevice &D = g_static_dev[dev];
+        if (!D.ready) {
+            // set-up, once per device, with that device current: the device address of the static array
+            void *p = nullptr;
+            STATIC_CUDA(cudaGetSymbolAddress(&p, g_static_scratch));
+            STATIC_CUDA(cudaDeviceGetAttribute(&D.sm_count, cudaDevAttrMultiProcessorCount, dev));
+            D.base = static_cast<unsigned char *>(p);
+            D.ready = true;
+        }
+        base = D.base;
+        sm_count = D.sm_count;
+        StaticScale &Sc = g_static_scale;
+        if (!(Sc.valid && Sc.L == box_L && memcmp(Sc.aziz, aziz, sizeof(Sc.aziz)) == 0)) {
+            Sc.scale = e32::aziz_f32_scale(G.az);
+            memcpy(Sc.aziz, aziz, sizeof(Sc.aziz));
+            Sc.L = box_L;
+            Sc.valid = true;
+        }
+        f32_scale = Sc.scale;
+    }
+    G.az.f32_scale = f32_scale;
+
+    GroupDev *groups = reinterpret_cast<GroupDev *>(base);
+    int32_t *group_of = reinterpret_cast<int32_t *>(base + kStaticGroupOfOff);
+    int32_t *enc = reinterpret_cast<int32_t *>(base + kStaticEncOff);
+    double *S = reinterpret_cast<double *>(base + kStaticSOff);
+    double *epart = reinterpret_cast<double *>(base + kStaticPartOff);
+
+    // the split of a walker over thread blocks, as plan_energy_f32g chooses it
+    const int nblk = (int)(NP >> 5);
+    int parts = (4 * sm_count + W - 1) / W;
+    const int max_parts = (nblk + 7) / 8;
+    if (parts > max_parts) parts = max_parts;
+    if (parts < 1) parts = 1;
+
+    StateView sv{};
+    sv.pos = nullptr;                       // the gridded kernels read the fixed-point copy only
+    sv.S = S;
+    sv.n_acc = nullptr;
+    sv.group_of = group_of;
+    sv.groups = groups;
+    sv.W = W; sv.N = N; sv.ld = (N + 3) & ~3;
+    sv.walker_id_base = 0;
+    sv.proposal = 0;
+
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    static_tables_kernel<<<(W + 255) / 256, 256, 0, st>>>(G, groups, group_of, W);
+    encode_angstrom_kernel<<<dim3((unsigned)W, (unsigned)((NP + 127) / 128)), 128, 0, st>>>(d_xyz, N, (int)NP, box_L, enc);
+    energy32g_kernel<256, true><<<(unsigned)W * (unsigned)parts, 256, 0, st>>>(sv, enc, (int)NP, parts, epart);
+    finalize32g_kernel<<<(W + 127) / 128, 128, 0, st>>>(sv, hbar2_over_2m, epart, parts, d_out);
+    STATIC_CUDA(cudaGetLastError());
+#undef STATIC_CUDA
+    return QMC_OK;
+}
