@@ -90,7 +90,12 @@ struct HistCtx {
 // Two pairs per lane (particles j, j + 1: the same two j for all lanes) in packed fp32; kMask: some lanes hold no
 // valid pair.  A pair that is clear of every bin edge and of the cutoff is counted at once (predicated shared-memory
 // reduction: a branch around atomicAdd costs BSSY / BRA / BSYNC per pair; Hs = shared-window address of bin 0 minus
-// 4 x 0x4B000000); slow = true: the pair needs the specified arithmetic.  sqrt(0) = 0 lands in the guard band of bin 0.
+// 4 x 0x4B400000); slow = true: the pair needs the specified arithmetic.
+// floor(v) is read from the low bits of fl((v - 1/2) + 1.5 x 2^23).  The constant is 1.5 x 2^23 and not 2^23 because
+// v - 1/2 is NEGATIVE for v < 1/2: 2^23 plus a negative number falls into the binade below 2^23, where the fp32 spacing
+// is 1/2, and reads as bin -1 (round 2 did that for every pair closer than a quarter bin).  Around 1.5 x 2^23 the
+// spacing is 1 on both sides: u - guard - 1/2 < -1/2 rounds to -1 and u + guard - 1/2 to 0, so a pair with u < guard
+// (r = 0 included) differs in the two estimates and takes the specified arithmetic like any pair next to a bin edge.
 template <bool kMask>
 __device__ __forceinline__ void hist_pair2(const HistCtx &C, int32_t xi, int32_t yi, int32_t zi, int32_t X0, int32_t X1,
                                            int32_t Y0, int32_t Y1, int32_t Z0, int32_t Z1, bool valid0, bool valid1,
@@ -104,10 +109,10 @@ __device__ __forceinline__ void hist_pair2(const HistCtx &C, int32_t xi, int32_t
     upk2(r2, ra, rb);
     asm("sqrt.approx.ftz.f32 %0, %0;" : "+f"(ra));
     asm("sqrt.approx.ftz.f32 %0, %0;" : "+f"(rb));
-    const f32x2 rr = pk2(ra, rb), us = pk1(C.uscale), magic = pk1(8388608.0f);
+    const f32x2 rr = pk2(ra, rb), us = pk1(C.uscale), magic = pk1(12582912.0f);
     float l0, l1, h0, h1;
-    upk2(add2(fma2(rr, us, pk1(C.lo_off)), magic), l0, l1);           // 2^23 + floor(u - guard), both pairs
-    upk2(add2(fma2(rr, us, pk1(C.hi_off)), magic), h0, h1);           // 2^23 + floor(u + guard)
+    upk2(add2(fma2(rr, us, pk1(C.lo_off)), magic), l0, l1);           // 1.5 x 2^23 + floor(u - guard), both pairs
+    upk2(add2(fma2(rr, us, pk1(C.hi_off)), magic), h0, h1);           // 1.5 x 2^23 + floor(u + guard)
     const int a0 = __float_as_int(l0), a1 = __float_as_int(l1), b0 = __float_as_int(h0), b1 = __float_as_int(h1);
     slow0 = a0 != b0;
     slow1 = a1 != b1;
@@ -160,11 +165,11 @@ __global__ void __launch_bounds__(256, 4) pair_histogram_kernel(StateView sv, in
     const double inv_dr = __ddiv_rn((double)nbins, h);
     HistCtx C;
     C.H = H; C.Q = Qall + warp * kQueue; C.cnt = 0;
-    C.Hs = (uint32_t)__cvta_generic_to_shared(H) - 4u * 0x4B000000u;
+    C.Hs = (uint32_t)__cvta_generic_to_shared(H) - 4u * 0x4B400000u;
     C.uscale = (float)nbins * 0x1p-31f;                               // u = (r / L) 2 nbins, r / L arrives times 2^32
-    // floor(v) for 0 <= v < 2^22 not within rounding of an integer: the low bits of fl((v - 1/2) + 2^23)
+    // floor(v) for -1/2 <= v < 2^22 not within rounding of an integer: the low bits of fl((v - 1/2) + 1.5 x 2^23)
     C.lo_off = -(0.5f + kGuard); C.hi_off = -(0.5f - kGuard);
-    C.in_limit = 0x4B000000 + nbins;                                  // bit pattern of 2^23 + nbins
+    C.in_limit = 0x4B400000 + nbins;                                  // bit pattern of 1.5 x 2^23 + nbins
     // pairs that need the specified arithmetic wait in the warp's queue and are evaluated 32 at a time, one per
     // lane: the fp64 code never runs with a few lanes of a warp only
     auto drain = [&](int first, int n) {                              // entries [first, first + n), n <= 32
