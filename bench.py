@@ -32,9 +32,23 @@ from paper_1312_1282_b200 import workloads as wl  # noqa: E402
 # checked against ncu's sm__sass_thread_inst_executed_op_* per executed pair evaluation in profiles/r02_instr.md.
 ALG_INSTR = {wl.MODE_FP32C: 24.0, wl.MODE_FP64: 31.0}
 LANES_PER_SM = {wl.MODE_FP32C: 128, wl.MODE_FP64: 64}
-# DRAM bytes per launch of the dominant kernel from the ncu --set full capture of the same command
-# (profiles/r02b_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum); None where no capture exists.
+# SURVEY.md section 8(d)'s own estimate of the same count for the FP32C pair term (a second reading of "algorithmic")
+SURVEY_INSTR_FP32C = 28.0
+# DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum).  These are NOT measured
+# by this run: they are typed in from the ncu --set full capture of this command that profiles/r02b_kernels.md
+# summarises (round-2 sweep kernels, unchanged since; 2048 walkers of 1952 atoms).  None where no capture exists.
+# `traffic_compulsory` in the JSON line is computed from W, N and the mode instead.
 NCU_TRAFFIC_BYTES = {("c3-N1952", wl.MODE_FP32C): 80.0e6 + 22.4e6, ("c3-N1952-fp64", wl.MODE_FP64): 129.7e6 + 70.4e6}
+NCU_TRAFFIC_SOURCE = "profiles/r02b_kernels.md (ncu --set full of this command, round-2 kernels; a constant, not measured by this run)"
+# Issue slots per EXECUTED pair evaluation of the FP32C sweep on each pipe, in thread terms (warp instructions x 32 /
+# executed pair evaluations), and ncu's pipe utilisation of the same launch: profiles/r02b_instr.md and
+# profiles/r02b_kernels.md (sweep_kernel<float, 128, 16, 4, 1, 0>, 2048 x 1952, acceptance 0.523).  Constants from
+# those files, quoted so that the pipe bound below can be recomputed by a reader.
+NCU_SWEEP32_SLOTS = {"issue": 19.36, "fma": 6.23, "alu": 7.89, "xu": 2.26, "fp64": 0.55, "lsu": 2.03}
+NCU_SWEEP32_UTIL_PCT = {"pipe_fma": 37.7, "pipe_xu": 57.8, "pipe_alu": 51.4, "issue_active": 61.9}
+# thread-level instructions per SM and clock each pipe can take (guide: 4 schedulers x 1 warp instruction per clock;
+# FMA 128 lanes, of which a packed FFMA2 holds its lane for two clocks -- profiles/r01_pipes.md; ALU 64; XU 16; FP64 64)
+PIPE_LANES = {"issue": 128.0, "fma": 128.0, "alu": 64.0, "xu": 16.0, "fp64": 64.0, "lsu": 32.0}
 EQUIL_SWEEPS = {1: 200, 2: 200, 3: 150, 4: 20, 5: 60}      # untimed, before the warm-up (time the liquid, not the melting lattice)
 
 
@@ -97,9 +111,38 @@ def cpu_baseline(w: wl.Workload, m: int, budget_s: float = 12.0):
         if el >= budget_s or steps >= 50:
             break
     pairs = steps * cores * (m * N * (N - 1) + N * (N - 1) // 2)
+    # ONE core, as the paper's CPU column is ("a single-core CPU execution"): a single walker, which
+    # the oracle runs on one thread (it parallelises over walkers only)
+    x1 = x[:1].copy()
+    n1, t1 = 0, time.perf_counter()
+    while True:
+        oracle.sweep(s, x1, w.seed, 0, t, m, g.step)
+        oracle.local_energy(s, x1)
+        t += m
+        n1 += 1
+        el1 = time.perf_counter() - t1
+        if el1 >= min(3.0, budget_s / 4) or n1 >= 20:
+            break
+    pairs_step_walker = m * N * (N - 1) + N * (N - 1) // 2
+    single = n1 * pairs_step_walker / el1
+    full_pairs = w.n_walkers * w.sweeps * (N * (N - 1) + N * (N - 1) // 2)       # BASELINE.json: energy every sweep
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for ln in fh:
+                if ln.startswith("model name"):
+                    model = ln.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
     return {"value": pairs / el, "unit": "pair-evals/s", "cores": cores, "kind": "oracle",
             "sample": f"{cores} walkers x {steps} steps (m={m} sweeps + 1 energy) of {w.name}, fp64, {el:.1f} s wall",
-            "walker_sweeps_per_s": steps * cores * m / el, "ms_per_step_sample": 1e3 * el / steps}
+            "walker_sweeps_per_s": steps * cores * m / el, "ms_per_step_sample": 1e3 * el / steps,
+            "cpu_model": model,
+            "single_core_pair_evals_per_s": single,
+            "single_core_sample": f"1 walker x {n1} steps on one thread, {el1:.1f} s wall",
+            "full_config_seconds_extrapolated": {"all_cores": full_pairs / (pairs / el), "single_core": full_pairs / single,
+                                                 "of": f"{w.n_walkers} walkers x {w.sweeps} sweeps, energy every sweep"}}
 
 
 def run_reference(args, w, m):
@@ -216,8 +259,10 @@ class Timed:
         self.launches = q.info()["kernel_launches"] - launches0
         if barrier:
             barrier()
-        self.t_sweep = sum(ev[k][0].elapsed_time(ev[k][1]) for k in range(K)) * 1e-3
-        self.t_total = sum(ev[k][0].elapsed_time(ev[k][2]) for k in range(K)) * 1e-3
+        self.sweep_ms = [ev[k][0].elapsed_time(ev[k][1]) for k in range(K)]
+        self.step_ms = [ev[k][0].elapsed_time(ev[k][2]) for k in range(K)]
+        self.t_sweep = sum(self.sweep_ms) * 1e-3
+        self.t_total = sum(self.step_ms) * 1e-3
         self.acc = float(self.a_out.mean())
         self.e_mean = (self.e_out.mean(0) / self.w.n_atoms).tolist()
         return self
@@ -235,6 +280,7 @@ def summarize(t: "Timed", K, sm_count, sm_max_mhz, world=1):
         "workload": w.name, "N": w.n_atoms, "walkers": w.n_walkers, "groups": len(w.groups),
         "mode": "fp32c" if w.mode == wl.MODE_FP32C else "fp64", "steps": K,
         "ms_per_step": 1e3 * t.t_total / K, "sweep_ms": 1e3 * t.t_sweep / K, "energy_ms": 1e3 * (t.t_total - t.t_sweep) / K,
+        "ms_per_step_median": statistics.median(t.step_ms), "sweep_ms_median": statistics.median(t.sweep_ms),
         "pair_evals_per_s": world * K * (sweep_pairs + energy_pairs) / t.t_total,
         "sweep_pair_evals_per_s": world * K * sweep_pairs / t.t_sweep,
         "energy_pairs_per_s": world * K * energy_pairs / (t.t_total - t.t_sweep),
@@ -264,9 +310,10 @@ def main():
                     help="0: particles in order, uniform cube (BASELINE.json); 1: the paper's random particle + "
                          "Gaussian displacement (NEXT-1), standard deviation --sigma per component")
     ap.add_argument("--sigma", type=float, default=0.8, help="proposal 1: standard deviation per component, Angstrom")
-    ap.add_argument("--time-to-error", type=int, default=0, metavar="S",
+    ap.add_argument("--time-to-error", type=int, default=None, metavar="S",
                     help="after the timed steps: S more steps with the energy recorded, reblocked -> the paper's "
-                         "t*sigma^2 and seconds to 1 mK per atom (PAPER.md l.504-511); 0 = skip")
+                         "t*sigma^2 and seconds to 1 mK per atom (PAPER.md l.504-511); 0 = skip; default 40 for the "
+                         "headline config on one GPU (under a second), else 0")
     ap.add_argument("--large-n", action="store_true", help="add the NEXT-3 cluster-kernel figures (N = 40960, one walker on 8 SMs)")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
                     help="qmc_set_tuning override for the headline workload, e.g. --tune sweep_tile=4 (tuning experiments; "
@@ -371,14 +418,50 @@ def main():
     t_launch = t_sweep / K
     achieved = sweep_pairs * ALG_INSTR[w.mode] / t_launch
     executed = sweep_pairs * (1.0 + acc) * ALG_INSTR[w.mode] / t_launch
-    traffic = NCU_TRAFFIC_BYTES.get((w.name, w.mode)) if m == 1 else None
+    traffic = NCU_TRAFFIC_BYTES.get((w.name, w.mode)) if m == 1 and not args.walkers else None
+    real_bytes = 8 if w.mode == wl.MODE_FP64 else 4
+    ld = (N + 3) // 4 * 4
+    # algorithmic bytes of one sweep launch: coordinates and running sums read once and written once, counters (the
+    # written half may still sit in the 126 MB L2 when the launch ends, which is why ncu's dram figure can be lower)
+    traffic_algorithmic = 2 * (W * 3 * ld * real_bytes + W * ld * 8) + 2 * W * 8
+    # Lower bound of the FP32C sweep's time from the MEASURED instruction mix (ncu, per executed pair evaluation) and
+    # the pipes' rates: every pipe must at least issue its own instructions; the largest of these is the bound.
+    pipe_bound = None
+    if w.mode == wl.MODE_FP32C and w.name == "c3-N1952":
+        clk = sm_max * 1e6
+        executed_pairs = sweep_pairs * (1.0 + acc)
+        ffma2_lane_rate = 2.0 * rates["ffma2"]                                    # fp32 lane results per second, packed
+        per_pipe = {}
+        for pipe, slots in NCU_SWEEP32_SLOTS.items():
+            rate = info["sm_count"] * PIPE_LANES[pipe] * clk                      # thread-instr/s the pipe can issue
+            if pipe == "xu":
+                rate = min(rate, rates["mufu_rsq"])                               # live probe
+            per_pipe[pipe] = {"slots_per_executed_pair": slots, "rate_G_s": rate / 1e9,
+                              "t_min_ms": 1e3 * slots * executed_pairs / rate}
+        # the FMA pipe's packed instructions occupy it for two clocks: its bound in pipe-cycles is what ncu's
+        # pipe_fma_cycles_active measures
+        per_pipe["fma"]["t_min_ms_packed_two_clocks"] = 2.0 * per_pipe["fma"]["t_min_ms"]
+        bound_pipe = max(per_pipe, key=lambda k: per_pipe[k]["t_min_ms"])
+        t_bound = per_pipe[bound_pipe]["t_min_ms"]
+        pipe_bound = {"per_pipe": per_pipe, "binding_pipe": bound_pipe, "t_bound_ms": t_bound,
+                      "frac_of_pipe_bound": t_bound / (1e3 * t_launch),
+                      "ncu_utilization_pct": NCU_SWEEP32_UTIL_PCT, "ffma2_lane_rate_measured_G_s": ffma2_lane_rate / 1e9,
+                      "source": "instruction mix: profiles/r02b_instr.md; utilisation: profiles/r02b_kernels.md (constants of the "
+                                "round-2 sweep kernel, unchanged this round); rates: SMs x lanes x max clock, XU from the live probe",
+                      "reading": "no pipe is saturated: the issue slots are the tightest bound, and the kernel runs at "
+                                 "frac_of_pipe_bound of it; the rest is the per-move serial part (reduction, barrier, decision)"}
     roofline = {
         "bound": "alu", "kernel": f"sweep_kernel<{mode_name}>",
         "achieved": achieved / 1e9, "peak": peak_derived / 1e9, "unit": "G thread-instr/s",
         "frac": achieved / peak_derived, "traffic": traffic,
-        "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum per launch, ncu --set full of this command "
-                        "(profiles/r02b_kernels.md); the walker state is 80 MB (fp32c) / 128 MB (fp64): read once, "
-                        "coordinates + S written once",
+        "traffic_source": NCU_TRAFFIC_SOURCE if traffic is not None else None,
+        "traffic_algorithmic": traffic_algorithmic,
+        "traffic_note": "traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch from the named ncu capture; "
+                        "traffic_algorithmic: computed here from W, N and the mode (coordinates + running sums read once "
+                        "and written once; written lines may outlive the launch in L2)",
+        "frac_survey_count": (sweep_pairs * SURVEY_INSTR_FP32C / t_launch / peak_derived) if w.mode == wl.MODE_FP32C else None,
+        "frac_of_measured_fma_chain": achieved / peak_meas,
+        "pipe_bound": pipe_bound,
         "peak_source": f"derived: {info['sm_count']} SMs x {LANES_PER_SM[w.mode]} lanes x {sm_max:.0f} MHz (DESIGN.md); "
                        "MEASURED_PEAKS.json has no ALU entry",
         "peak_measured_fma_chain": peak_meas / 1e9,
@@ -399,6 +482,7 @@ def main():
         "metric": "pair evaluations/s (sweep N(N-1) + energy N(N-1)/2 per walker-step)",
         "value": value, "unit": "pair-evals/s", "n_gpus": world, "steps": K, "warmup": args.warmup,
         "ms_per_step": 1e3 * t_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step_median": statistics.median(head.step_ms), "sweep_ms_median": statistics.median(head.sweep_ms),
         "dtype": "f32" if w.mode == wl.MODE_FP32C else "f64", "data": "synthetic",
         "config": {"workload": w.name, "N": N, "walkers_per_gpu": W, "groups": len(w.groups),
                    "sweeps_per_step": m, "mode": mode_name, "energy_every_step": True,
@@ -449,9 +533,15 @@ def main():
     e_out = head.e_out
     # ---- observables beside the hot path: g(r) histogram, time to error ----
     nb = 256
-    if 24 * N + 4 * nb <= 227 * 1024:
-        hist = torch.empty((W, nb), dtype=torch.int32, device=dev)
+    hist = torch.empty((W, nb), dtype=torch.int32, device=dev)
+    try:
         q.pair_histogram(nb, hist)
+        hist_ok = True
+    except binding.QmcError as exc:                  # QMC_E_CAPACITY: N beyond that kernel's shared memory
+        if exc.code != binding.QMC_E_CAPACITY:
+            raise
+        hist_ok = False
+    if hist_ok:
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
@@ -493,6 +583,8 @@ def main():
                                      "host memory every m sweeps and raise per-walker flags)"}
     if args.large_n:
         out["large_n"] = large_n_block(dev, flush)
+    if args.time_to_error is None:
+        args.time_to_error = 40 if (args.config == 3 and world == 1 and not args.walkers) else 0
     if args.time_to_error > 0:
         from paper_1312_1282_b200 import observables as ob
         S = args.time_to_error
@@ -507,6 +599,8 @@ def main():
         tsig, t_goal = ob.seconds_to_error(se, el)
         out["time_to_error"] = {"steps": S, "seconds": el, "E_per_atom_K": mean, "se_K": se, "tau_steps": tau,
                                 "t_sigma2_s_mK2": tsig, "seconds_to_1mK_per_atom": t_goal,
+                                "paper_t_sigma2_s_mK2": {"N512_K20": 130.0, "N512_M2090": 200.0,
+                                                         "cite": "PAPER.md l.504-511 (other hardware, N = 512: context only)"},
                                 "note": f"chain equilibrated for {equil}+ sweeps before the series"}
     if not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w, m)

@@ -106,7 +106,9 @@ int qmc_local_energy(qmc_ctx *c, double *d_out);
  * 1 <= nbins <= 8192; QMC_E_CAPACITY if 12 N + 4 nbins + 5 KB exceed one CTA's shared memory (N <= ~18 000). */
 int qmc_pair_histogram(qmc_ctx *c, int32_t nbins, uint32_t *d_hist);
 
-/* d_out: device [W] accepted / attempted moves since qmc_init_walkers / qmc_set_positions. */
+/* Acceptance ratio, one of the quantities the paper writes out with every block (l.323, l.381; its file
+ * acceptance.dat, l.397-406): d_out: device [W] accepted / attempted moves since qmc_init_walkers /
+ * qmc_set_positions. */
 int qmc_acceptance(qmc_ctx *c, double *d_out);
 
 /* One whole step with HOST buffers (the paper's block cycle, l.319-343: coordinates in, sweeps, energies and
@@ -181,8 +183,16 @@ typedef struct {
 } qmc_info_t;
 int qmc_info(const qmc_ctx *c, qmc_info_t *out);
 
-/* Process-wide override of the launch heuristics for the contexts created AFTERWARDS (tuning experiments and
- * tests; the defaults are what bench.py times).  Keys: "sweep_threads", "sweep_per_thread", "sweep_vector",
+/* qmc_create with this context's own overrides of the launch heuristics: n_keys (key, value) pairs with the keys listed
+ * under qmc_set_tuning below; everything not named is left to the heuristics, and the process-wide defaults of
+ * qmc_set_tuning are NOT consulted.  Contexts with different forced shapes can coexist and be created from different
+ * threads.  keys / values: host arrays, read during the call only.  QMC_E_ARG for an unknown key. */
+int qmc_create_tuned(const qmc_params *p, void *cuda_stream, void *d_state, size_t state_bytes,
+                     const char *const *keys, const int32_t *values, int32_t n_keys, qmc_ctx **out);
+
+/* Process-wide DEFAULT of those overrides: copied into a context by qmc_create at creation (later changes do not reach
+ * it) and ignored by qmc_create_tuned.  A plain global without a lock -- for single-threaded tuning experiments and
+ * tests; use qmc_create_tuned otherwise.  The heuristics themselves (no override) are what bench.py times.  Keys: "sweep_threads", "sweep_per_thread", "sweep_vector",
  * "sweep_pending", "sweep_tile" (1 = one-move kernel, 2 / 4 = tile kernel), "sweep_cluster", "energy_threads",
  * "energy_ordered" (1 = ordered-pair energy kernels), "host_chunks" (walker chunks of qmc_step_host, 1..8).  value: the wanted number, or -1 (0 for the energy keys) for
  * "heuristic".  key == NULL resets everything.  A shape that is not compiled or does not fit N falls back to the

@@ -22,7 +22,7 @@ EXPORTS = (
     "qmc_acceptance", "qmc_step_host", "qmc_last_error", "qmc_get_positions", "qmc_set_positions",
     "qmc_set_seed", "qmc_get_pair_sums", "qmc_refresh_pair_sums", "qmc_trace_decisions", "qmc_info",
     "qmc_pair_histogram", "qmc_set_proposal", "qmc_run_blocks_host", "qmc_wait", "qmc_sweep_writeouts",
-    "qmc_set_tuning", "qmc_local_energy_fp32c_static",
+    "qmc_set_tuning", "qmc_local_energy_fp32c_static", "qmc_create_tuned",
 )
 # limits of qmc_local_energy_fp32c_static (include/qmc.h)
 STATIC_MAX_WALKERS, STATIC_MAX_ATOMS, STATIC_MAX_SLOTS, STATIC_SCRATCH_BYTES = 4096, 65536, 262144, 5382656
@@ -78,6 +78,8 @@ def load_library() -> C.CDLL:
     lib.qmc_state_bytes.argtypes = [C.POINTER(_Params)]
     lib.qmc_state_bytes.restype = C.c_size_t
     lib.qmc_create.argtypes = [C.POINTER(_Params), vp, vp, C.c_size_t, C.POINTER(vp)]
+    lib.qmc_create_tuned.argtypes = [C.POINTER(_Params), vp, vp, C.c_size_t, C.POINTER(C.c_char_p), C.POINTER(C.c_int32),
+                                     C.c_int32, C.POINTER(vp)]
     lib.qmc_destroy.argtypes = [vp]
     lib.qmc_init_walkers.argtypes = [vp, C.c_uint64]
     lib.qmc_sweep.argtypes = [vp, C.c_int32, dp]
@@ -189,7 +191,9 @@ class QMC:
     def __init__(self, N: int, walkers_per_group: Sequence[int], box_L: Sequence[float],
                  jastrow_b: Sequence[float], hbar2_over_2m: float, aziz: Sequence[float], mode: int,
                  walker_id_base: int = 0, jitter: float = 0.05, device: str = "cuda:0", stream=None,
-                 library_owns_state: bool = False):
+                 library_owns_state: bool = False, tuning: Optional[dict] = None):
+        """tuning: this context's own launch overrides ({"sweep_threads": 128, ...}, the keys of qmc_set_tuning) through
+        qmc_create_tuned; None: qmc_create, which takes the process-wide defaults of set_tuning()."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1312_1282_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
@@ -209,14 +213,19 @@ class QMC:
             raise QmcError(QMC_E_ARG, "invalid parameters")
         self._ctx = C.c_void_p()
         if library_owns_state:
-            self._state = None
-            rc = self._lib.qmc_create(C.byref(self._params), C.c_void_p(self.stream.cuda_stream), None, 0,
-                                      C.byref(self._ctx))
+            self._state, base, given = None, None, 0
         else:
             self._state = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-            base = (self._state.data_ptr() + 255) & ~255
-            rc = self._lib.qmc_create(C.byref(self._params), C.c_void_p(self.stream.cuda_stream),
-                                      C.c_void_p(base), nbytes, C.byref(self._ctx))
+            base, given = C.c_void_p((self._state.data_ptr() + 255) & ~255), nbytes
+        if tuning is None:
+            rc = self._lib.qmc_create(C.byref(self._params), C.c_void_p(self.stream.cuda_stream), base, given,
+                                      C.byref(self._ctx))
+        else:
+            n = len(tuning)
+            keys = (C.c_char_p * max(n, 1))(*[k.encode() for k in tuning])
+            vals = (C.c_int32 * max(n, 1))(*[int(v) for v in tuning.values()])
+            rc = self._lib.qmc_create_tuned(C.byref(self._params), C.c_void_p(self.stream.cuda_stream), base, given,
+                                            keys, vals, n, C.byref(self._ctx))
         if rc != 0:
             self._ctx = C.c_void_p()
             raise QmcError(rc, self._lib.qmc_last_error(None).decode())

@@ -254,13 +254,45 @@ extern "C" size_t qmc_state_bytes(const qmc_params *p)
     return tot;
 }
 
+static bool tuning_set(Tuning &t, const char *key, int32_t value)
+{
+    struct { const char *name; int *field; } tab[] = {
+        {"sweep_threads", &t.sweep_threads}, {"sweep_per_thread", &t.sweep_per_thread}, {"sweep_vector", &t.sweep_vector},
+        {"sweep_pending", &t.sweep_pending}, {"sweep_tile", &t.sweep_tile}, {"sweep_cluster", &t.sweep_cluster},
+        {"energy_threads", &t.energy_threads}, {"energy_ordered", &t.energy_ordered}, {"host_chunks", &t.host_chunks},
+    };
+    for (auto &e : tab)
+        if (strcmp(key, e.name) == 0) { *e.field = value; return true; }
+    return false;
+}
+
+static int create_impl(const qmc_params *p, void *cuda_stream, void *d_state, size_t state_bytes, const Tuning &tuning, qmc_ctx **out);
+
 extern "C" int qmc_create(const qmc_params *p, void *cuda_stream, void *d_state, size_t state_bytes, qmc_ctx **out)
+{
+    return create_impl(p, cuda_stream, d_state, state_bytes, g_tuning, out);
+}
+
+extern "C" int qmc_create_tuned(const qmc_params *p, void *cuda_stream, void *d_state, size_t state_bytes,
+                                const char *const *keys, const int32_t *values, int32_t n_keys, qmc_ctx **out)
+{
+    if (out) *out = nullptr;
+    if (n_keys < 0 || (n_keys > 0 && (!keys || !values))) QMC_FAIL((qmc_ctx *)nullptr, QMC_E_ARG, "qmc_create_tuned: keys and values are required");
+    Tuning t{};                                          // the heuristics, whatever qmc_set_tuning has been told
+    for (int k = 0; k < n_keys; ++k)
+        if (!keys[k] || !tuning_set(t, keys[k], values[k]))
+            QMC_FAIL((qmc_ctx *)nullptr, QMC_E_ARG, "qmc_create_tuned: unknown key '%s'", keys[k] ? keys[k] : "(null)");
+    return create_impl(p, cuda_stream, d_state, state_bytes, t, out);
+}
+
+static int create_impl(const qmc_params *p, void *cuda_stream, void *d_state, size_t state_bytes, const Tuning &tuning, qmc_ctx **out)
 {
     if (!out) QMC_FAIL((qmc_ctx *)nullptr, QMC_E_ARG, "out is NULL");
     *out = nullptr;
     if (!valid_params(p, g_create_err)) return QMC_E_ARG;
     qmc_ctx *c = new (std::nothrow) qmc_ctx();
     if (!c) QMC_FAIL((qmc_ctx *)nullptr, QMC_E_ARG, "out of host memory");
+    c->tuning = tuning;
     c->p = *p;
     c->walkers_per_group.assign(p->walkers_per_group, p->walkers_per_group + p->n_groups);
     c->box_L.assign(p->box_L, p->box_L + p->n_groups);
@@ -442,9 +474,9 @@ extern "C" int qmc_sweep(qmc_ctx *c, int32_t n_sweeps, const double *steps)
     }
     if (changed)   // stream-ordered update of the small constant table (host mirror is ours, pageable copy is synchronous to the host)
         QMC_CUDA(c, cudaMemcpyAsync(c->d_groups, c->groups.data(), sizeof(GroupDev) * c->p.n_groups, cudaMemcpyHostToDevice, c->stream));
-    if (c->sweep_plan.cluster > 1 && (c->sv.proposal != 0 || c->wo.xyz != nullptr))
-        QMC_FAIL(c, QMC_E_ARG, "the cluster sweep kernel (N = %d on %d blocks per walker) takes proposal 0 and no in-kernel write-outs",
-                 c->p.N, c->sweep_plan.cluster);
+    if (c->sweep_plan.cluster > 1 && c->sweep_plan.fallback == nullptr && (c->sv.proposal != 0 || c->wo.xyz != nullptr))
+        QMC_FAIL(c, QMC_E_ARG, "the cluster sweep kernel (N = %d on %d blocks per walker) takes proposal 0 and no in-kernel write-outs, "
+                 "and no single thread block can hold a walker of this size", c->p.N, c->sweep_plan.cluster);
     {
         NvtxRange r("qmc_sweep");
         QMC_CUDA(c, launch_sweep(c, n_sweeps));
@@ -616,7 +648,7 @@ extern "C" int qmc_step_host(qmc_ctx *c, const double *h_xyz_in, const double *h
     // run on three streams, so that chunk k+1 uploads and chunk k-1 downloads while chunk k computes; two compute
     // streams let the sweep of one chunk share the GPU with the energy pass of the previous one.  A decision trace
     // (walker indices of the whole context) or few walkers keep everything in one chunk.
-    int nchunk = g_tuning.host_chunks > 0 ? g_tuning.host_chunks : 4;
+    int nchunk = c->tuning.host_chunks > 0 ? c->tuning.host_chunks : 4;
     if (nchunk > kHostChunksMax) nchunk = kHostChunksMax;
     while (nchunk > 1 && (int)Wt / nchunk < c->sm_count) --nchunk;
     if (c->trace.dec) nchunk = 1;
@@ -755,15 +787,8 @@ extern "C" int qmc_info(const qmc_ctx *c, qmc_info_t *out)
 
 extern "C" int qmc_set_tuning(const char *key, int32_t value)
 {
-    Tuning &t = g_tuning;
-    if (!key) { t = Tuning{}; return QMC_OK; }
-    struct { const char *name; int *field; } tab[] = {
-        {"sweep_threads", &t.sweep_threads}, {"sweep_per_thread", &t.sweep_per_thread}, {"sweep_vector", &t.sweep_vector},
-        {"sweep_pending", &t.sweep_pending}, {"sweep_tile", &t.sweep_tile}, {"sweep_cluster", &t.sweep_cluster},
-        {"energy_threads", &t.energy_threads}, {"energy_ordered", &t.energy_ordered}, {"host_chunks", &t.host_chunks},
-    };
-    for (auto &e : tab)
-        if (strcmp(key, e.name) == 0) { *e.field = value; return QMC_OK; }
+    if (!key) { g_tuning = Tuning{}; return QMC_OK; }
+    if (tuning_set(g_tuning, key, value)) return QMC_OK;
     snprintf(g_create_err, 512, "qmc_set_tuning: unknown key '%s'", key);
     return QMC_E_ARG;
 }

@@ -208,7 +208,7 @@ bool plan_energy(qmc_ctx *c, EnergyPlan *out)
         // one walker per block while that fills the GPU; the gridded kernel for few walkers of many atoms (a block
         // per walker would leave SMs idle) and for N beyond one block's shared memory.
         // qmc_set_tuning("energy_ordered"): 0 heuristic, 1 ordered pairs, 2 unordered pairs, 3 gridded.
-        const int want = g_tuning.energy_ordered;
+        const int want = c->tuning.energy_ordered;
         const bool few = (long long)c->W * 2 < c->sm_count && c->p.N >= 1024;
         if (want == 3 || (want == 0 && few)) return plan_energy_f32g(c, out);
         if (want != 1 && plan_energy_f32s(c, out)) return true;
@@ -216,13 +216,13 @@ bool plan_energy(qmc_ctx *c, EnergyPlan *out)
         if (plan_energy_f32(c, out)) return true;
         return plan_energy_f32g(c, out);
     }
-    if (g_tuning.energy_ordered != 1 && plan_energy_f64(c, out)) return true;
+    if (c->tuning.energy_ordered != 1 && plan_energy_f64(c, out)) return true;
     out->variant = 0;
     const int N = c->p.N;
     int T = 32;
     while (T < N && T < 256) T *= 2;
-    if (g_tuning.energy_threads > 0) {
-        const int v = g_tuning.energy_threads;
+    if (c->tuning.energy_threads > 0) {
+        const int v = c->tuning.energy_threads;
         if (v >= 32 && v <= 1024 && (v & (v - 1)) == 0) T = v;
     }
     out->threads = T;

@@ -408,8 +408,8 @@ bool plan_energy_f32(qmc_ctx *c, EnergyPlan *out)
     int T = 32;
     while (T < N && T < 256) T *= 2;
     if (smem_bytes32(N) > 113 * 1024) T = 512;      // one CTA per SM (N = 10000): fill it with 16 warps
-    if (g_tuning.energy_threads > 0) {
-        const int v = g_tuning.energy_threads;
+    if (c->tuning.energy_threads > 0) {
+        const int v = c->tuning.energy_threads;
         if (v >= 32 && v <= 512 && (v & (v - 1)) == 0) T = v;
     }
     out->threads = T;

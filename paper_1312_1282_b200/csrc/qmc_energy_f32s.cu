@@ -29,9 +29,14 @@ using namespace e32;
 // fixed-point grids of the per-particle accumulators: 2^-24 of a pair-sum term (t/32) and of a gradient term
 // (gm/128 times the minimum image in box units; the terms arrive times 2^32)
 constexpr double kFixS = 0x1p24, kFixG = 0x1p-8;
-// bad: a partial sum that is not finite (two particles on one grid point) cannot be carried by a fixed-point number
-__device__ __forceinline__ long long fix_s(float v, bool &bad) { bad |= !(fabsf(v) <= 3.0e38f); return __float2ll_rn(v * 0x1p24f); }
-__device__ __forceinline__ long long fix_g(float v, bool &bad) { bad |= !(fabsf(v) <= 3.0e38f); return __float2ll_rn(v * 0x1p-8f); }
+// bad: a partial sum the fixed-point accumulator cannot carry -- not finite (two particles on one grid point), or so
+// large that a few of them would wrap the 56-bit hi:lo sum of a particle (|sum| < 2^55 units): anything
+// from 2^52 units up, i.e. |v| >= 2^28 for a pair-sum partial and 2^60 for a gradient partial.  A pair-sum partial
+// reaches 2^28 only with a pair closer than ~0.01 L (a liquid's nearest pairs, r > 0.04 L, give ~2^18), where the fp32
+// pair term has lost the rest of the sum anyway.  Eight such partials on ONE particle stay inside the range; more
+// would need nine partners of one particle within 0.01 L of it, in nine different blocks of 32.
+__device__ __forceinline__ long long fix_s(float v, bool &bad) { bad |= !(fabsf(v) < 0x1p28f); return __float2ll_rn(v * 0x1p24f); }
+__device__ __forceinline__ long long fix_g(float v, bool &bad) { bad |= !(fabsf(v) < 0x1p60f); return __float2ll_rn(v * 0x1p-8f); }
 // A 64-bit fixed-point accumulator is two 32-bit words, hi (signed, units of 2^24) and lo (unsigned): v = hi 2^24 +
 // lo with 0 <= lo < 2^24 is added by TWO native 32-bit shared-memory atomics (a 64-bit atomic add on shared memory is
 // a compare-and-swap loop).  A particle receives at most nblk + 1 <= 81 additions, so lo stays below 2^31 and no
@@ -205,9 +210,11 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
         A += nwarps;
         while (A >= nblk) { A -= nblk; ++k; }
     }
-    // a singular configuration: the pair sums come out as NaN, as they would from a floating-point accumulator (the
-    // energies below are not finite then anyway: the Laplacian and potential totals are floating point)
-    const double poison = __syncthreads_or(bad) ? __longlong_as_double(0x7ff8000000000000LL) : 0.0;
+    // a singular configuration: the pair sums come out as NaN, as they would from a floating-point accumulator (for
+    // coincident particles the energies below are not finite anyway: the Laplacian and potential totals are floating
+    // point); a pair so close that the fixed-point sums could wrap poisons the walker's pair sums, T_PB and E_PB the same way
+    // With b = 0 (free particles) every fixed-point sum is multiplied by exactly 0 downstream: nothing to flag.
+    const double poison = (__syncthreads_or(bad) && g.b5 != 0.0) ? __longlong_as_double(0x7ff8000000000000LL) : 0.0;
 
     double tG2 = 0.0;
     for (int i = tid; i < N; i += T) {
@@ -237,7 +244,8 @@ energy32s_kernel(StateView sv, double Dk, double *__restrict__ out)
                 const double T_JF = -0.5 * Dku * lam;
                 double *o = out + (size_t)w * 4;
                 const double V = c * g.az.f32_scale;                                     // the potential was summed in units of f32_scale K
-                o[0] = V + T_PB; o[1] = V; o[2] = T_PB; o[3] = T_JF;
+                // V and T_JF are floating-point totals of their own; T_PB holds |G_i|^2 from the fixed-point sums
+                o[0] = V + T_PB + poison; o[1] = V; o[2] = T_PB + poison; o[3] = T_JF;
             }
         }
     }
@@ -295,8 +303,8 @@ bool plan_energy_f32s(qmc_ctx *c, EnergyPlan *out)
     int T = 32;
     while (2 * T < N && T < 256) T *= 2;
     if (N >= 1536) T = 384;              // 24 warps per SM at 80 registers beat 16 at 128 (9.32 -> 9.12 ms at N = 1952)
-    if (g_tuning.energy_threads > 0) {
-        const int v = g_tuning.energy_threads;
+    if (c->tuning.energy_threads > 0) {
+        const int v = c->tuning.energy_threads;
         if (v >= 32 && v <= 512 && ((v & (v - 1)) == 0 || v == 384)) T = v;
     }
     out->threads = T;

@@ -405,6 +405,29 @@ double near_pair_fraction(const qmc_ctx *c)
     return 4.18879 * r * r * r / (Lmin * Lmin * Lmin);
 }
 
+// The pending-slot and queue forms (kPend 1, 2) leave the repulsive term and the damping out for x >= 3.  That is a
+// property of the CONSTANTS: with HFD-B(HE)'s the repulsive term is below 3e-15 of the dispersion sum there and
+// F = 1 beyond D = 1.4; qmc_params.aziz is the caller's, so the assumption is checked for the numbers supplied
+// (ADVICE r2): D <= 3, and A exp(-alpha x + beta x^2) below 1e-14 of |c6/x^6 + c8/x^8 + c10/x^10| at 65 points from
+// x = 3 to the cutoff of the largest box.  Anything else (a softer repulsion, a wider damping, no dispersion at all)
+// takes the in-place evaluation of both exponentials for every pair (kPend 0).
+bool far_terms_negligible(const qmc_ctx *c)
+{
+    const double *a = c->p.aziz;                         // eps, r_m, A, alpha, beta, c6, c8, c10, D
+    if (!(a[8] <= 3.0)) return false;
+    double Lmax = 0.0;
+    for (double L : c->box_L) Lmax = L > Lmax ? L : Lmax;
+    const double x_hi = fmax(3.0, 0.5 * Lmax / a[1]);
+    for (int k = 0; k <= 64; ++k) {
+        const double x = 3.0 + (x_hi - 3.0) * (double)k / 64.0;
+        const double w = 1.0 / (x * x);
+        const double disp = fabs(w * w * w * (a[5] + w * (a[6] + w * a[7])));
+        const double rep = fabs(a[2]) * exp(x * (a[4] * x - a[3]));
+        if (!(rep <= 1e-14 * disp)) return false;
+    }
+    return true;
+}
+
 // How the exponentials are evaluated: 1 (per-lane pending slot) while few pairs are near (N = 1952 at liquid density:
 // 3.3 %); 2 (warp queue) for smaller boxes if two CTAs with their queues still fit an SM (N = 512: 12.5 %, N = 256:
 // 25 %); 0 (in place) when most pairs are near anyway (N = 64).
@@ -413,6 +436,7 @@ cudaError_t launch64(qmc_ctx *c, double *d_out, bool energy)
 {
     const int smem = smem_bytes64(c->p.N);
     if (!energy) return launch64k<T, false, 0>(c, d_out, smem);
+    if (!far_terms_negligible(c)) return launch64k<T, true, 0>(c, d_out, smem);
     const double f = near_pair_fraction(c);
     const int qbytes = (T >> 5) * 2 * kQueue64 * 8;
     if (f < 0.05) return launch64k<T, true, 1>(c, d_out, smem);
@@ -453,8 +477,8 @@ bool plan_energy_f64(qmc_ctx *c, EnergyPlan *out)
     if (smem > 227 * 1024) return false;
     // measured (c2, c5, c3): 128 threads up to N ~ 1000 (N = 512: 13.6 ms against 13.9 with 256), 256 above
     int T = N <= 64 ? 32 : (N <= 128 ? 64 : (N <= 1024 ? 128 : 256));
-    if (g_tuning.energy_threads > 0) {
-        const int v = g_tuning.energy_threads;
+    if (c->tuning.energy_threads > 0) {
+        const int v = c->tuning.energy_threads;
         if (v >= 32 && v <= 512 && ((v & (v - 1)) == 0 || v == 384)) T = v;
     }
     const int nblk = (N + 31) >> 5;

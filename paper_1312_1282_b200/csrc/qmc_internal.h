@@ -43,7 +43,9 @@ struct WriteoutView {
 
 struct SweepPlan  { int threads, J, V, P, K, cluster, Nc, smem_bytes, ctas_per_sm; const void *shape;   // cluster > 1: blocks per walker, slices of Nc particles
                     const void *fallback; int fallback_smem; };   // fallback: one-move shape for what the tile kernel does not take
-// Process-wide overrides of the launch heuristics (qmc_set_tuning; tuning experiments and tests); -1 / 0 = heuristic.
+// Overrides of the launch heuristics; -1 / 0 = heuristic.  Each context carries its own copy (qmc_ctx::tuning), filled at
+// creation: from the caller's key/value list (qmc_create_tuned) or from the process-wide default that qmc_set_tuning edits
+// (qmc_create).  Nothing reads g_tuning after a context exists.
 struct Tuning { int sweep_threads = 0, sweep_per_thread = 0, sweep_vector = -1, sweep_pending = -1, sweep_tile = -1,
                     energy_threads = 0, energy_ordered = 0, sweep_cluster = -1, host_chunks = 0; };
 constexpr int kHostChunksMax = 8;
@@ -81,6 +83,7 @@ struct qmc_ctx {
     bool host_ready = false;
     qmc::TraceView trace{};
     qmc::WriteoutView wo{};                        // in-kernel write-outs of the running qmc_sweep_writeouts call
+    qmc::Tuning tuning{};                          // this context's overrides of the launch heuristics
     qmc::SweepPlan sweep_plan{};
     qmc::EnergyPlan energy_plan{};
     uint64_t seed = 0;

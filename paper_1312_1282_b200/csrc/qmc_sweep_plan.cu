@@ -15,8 +15,14 @@ cudaError_t launch_sweep(qmc_ctx *c, int n_sweeps)
     c->launches += 1;
     if (c->sweep_plan.cluster > 1) {                                 // one walker per thread-block cluster (NEXT-3)
         const ClusterShape *cs = static_cast<const ClusterShape *>(c->sweep_plan.shape);
-        if (cs == nullptr || c->sv.proposal != 0 || c->wo.xyz != nullptr || c->p.N < 3) return cudaErrorNotSupported;
-        return cs->launch(c, n_sweeps, c->sweep_plan.smem_bytes, c->sweep_plan.cluster, c->sweep_plan.Nc);
+        if (cs == nullptr || c->p.N < 3) return cudaErrorNotSupported;
+        if (c->sv.proposal == 0 && c->wo.xyz == nullptr)
+            return cs->launch(c, n_sweeps, c->sweep_plan.smem_bytes, c->sweep_plan.cluster, c->sweep_plan.Nc);
+        // proposal 1 and in-kernel write-outs exist in the one-block kernel only: where one block can hold the walker
+        // the plan carries that shape as its fallback (slower for few walkers, but it serves the call)
+        const SweepShape *fb = static_cast<const SweepShape *>(c->sweep_plan.fallback);
+        if (fb == nullptr) return cudaErrorNotSupported;
+        return fb->launch(c, n_sweeps, c->sweep_plan.fallback_smem);
     }
     const SweepShape *sh = static_cast<const SweepShape *>(c->sweep_plan.shape);
     int smem = c->sweep_plan.smem_bytes;
@@ -43,7 +49,7 @@ static bool plan_cluster(qmc_ctx *c, SweepPlan *out, int C)
         const ClusterShape &s = tab[k];
         if (s.T * s.J < Nc || s.smem > 227 * 1024) continue;
         if (mode != QMC_FP64 && N % s.V != 0) continue;
-        if ((g_tuning.sweep_threads > 0 && s.T != g_tuning.sweep_threads) || (g_tuning.sweep_per_thread > 0 && s.J != g_tuning.sweep_per_thread)) continue;
+        if ((c->tuning.sweep_threads > 0 && s.T != c->tuning.sweep_threads) || (c->tuning.sweep_per_thread > 0 && s.J != c->tuning.sweep_per_thread)) continue;
         const double cost = (double)s.T * ((double)s.J + (mode == QMC_FP64 ? 4.0 : 12.0)) * (s.V == 2 && mode != QMC_FP64 ? 1.12 : 1.0);
         if (cost < best_cost) { best_cost = cost; best = &s; }
     }
@@ -88,11 +94,27 @@ bool plan_sweep(qmc_ctx *c, SweepPlan *out)
         if (s.K > 1 && (N % s.K != 0 || N < 2 * s.K)) return false;
         return s.smem <= 227 * 1024;
     };
-    const Tuning &tu = g_tuning;
+    const Tuning &tu = c->tuning;
     out->cluster = 1; out->Nc = 0;
+    // the one-block, one-move shape the heuristic would take: what a cluster plan falls back to for proposal 1 and
+    // in-kernel write-outs (nullptr when no single block holds the walker)
+    auto one_block = [&](int *smem) -> const SweepShape * {
+        const SweepShape *b = nullptr;
+        double b_cost = 1e300;
+        for (int k = 0; k < n; ++k) {
+            const SweepShape &s = tab[k];
+            if (!usable(s) || s.K > 1) continue;
+            double cost = shape_cost(s, N, W, mode, c->sm_count, s.occupancy(s.smem));
+            if (mode != QMC_FP64) cost *= (s.V == 4 ? 1.0 : (s.V == 2 ? 1.12 : 1.6)) * (s.P ? 1.0 : 1.06);
+            else                  cost *= (s.V == 2 ? 1.0 : 1.05);
+            if (cost < b_cost) { b_cost = cost; b = &s; }
+        }
+        *smem = b ? b->smem : 0;
+        return b;
+    };
     if (tu.sweep_cluster > 1 && N >= 3) {
         int C = tu.sweep_cluster > kClusterMax ? kClusterMax : tu.sweep_cluster;
-        if (plan_cluster(c, out, C)) return true;
+        if (plan_cluster(c, out, C)) { out->fallback = one_block(&out->fallback_smem); return true; }
     }
     auto wanted = [&](const SweepShape &s) {
         return (tu.sweep_threads <= 0 || s.T == tu.sweep_threads) && (tu.sweep_per_thread <= 0 || s.J == tu.sweep_per_thread)
@@ -130,7 +152,7 @@ bool plan_sweep(qmc_ctx *c, SweepPlan *out)
         c_few = W <= 16 ? 8 : (W <= 32 ? 4 : (W <= 64 ? 2 : 1));
     if (!best || c_few > 1) {                        // ... or no single block holds the walker: the smallest cluster that does
         for (int C = (best ? c_few : 2); C <= kClusterMax && N >= 3; C *= 2)
-            if (C >= c_few && plan_cluster(c, out, C)) return true;
+            if (C >= c_few && plan_cluster(c, out, C)) { out->fallback = one_block(&out->fallback_smem); return true; }
         if (!best) return false;
         out->cluster = 1; out->Nc = 0;
     }

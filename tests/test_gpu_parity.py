@@ -92,12 +92,47 @@ def test_init_walkers_fp32c_is_the_rounded_lattice(qmc, oracle):
     assert np.abs(d).max() < 0.51 * L / 2 ** 23
 
 
+def test_set_positions_fp32c_rounds_off_grid_input_to_the_nearest_grid_point(qmc, oracle):
+    """coordinates that are NOT on the FP32C grid (multiples of L 2^-23), and some outside [0, L):
+    stored as the nearest grid point of the wrapped value (|error| <= L 2^-24), and the energy of what is stored
+    equals the oracle's on the exported coordinates."""
+    N, W = 300, 2
+    q, L = make(qmc, N, W, qmc.QMC_FP32C)
+    x = np.stack([wl.liquid_configuration(N, L, 50 + k) for k in range(W)])          # fp64 uniform: off the grid
+    x[:, :, ::9] += L
+    x[:, :, 4::13] -= L
+    q.set_positions(x)
+    xs = q.get_positions().cpu().numpy()
+    k = xs / L * 2 ** 23
+    assert np.abs(k - np.rint(k)).max() < 1e-6 and k.min() > -1e-6 and k.max() < 2 ** 23    # (s - 1) L is rounded once
+    d = xs - x
+    d -= L * np.rint(d / L)
+    assert np.abs(d).max() <= L * 2.0 ** -24 * (1 + 1e-9)
+    assert np.abs(d).max() > L * 2.0 ** -26                                       # the input really was off the grid
+    eg = q.local_energy().cpu().numpy()
+    eo = oracle.local_energy(orc_sys(oracle, N, L), xs)
+    assert relerr32(eg, eo).max() < TOL32
+
+
 # ------------------------------------------------------------------------------ trajectories
+def check_shape(inf, tune):
+    """The forced shape exists and is the one that runs."""
+    for key, name in (("sweep_threads", "sweep_threads"), ("sweep_per_thread", "sweep_pairs_per_thread"),
+                      ("sweep_vector", "sweep_vector"), ("sweep_tile", "sweep_tile"), ("sweep_cluster", "sweep_cluster")):
+        if key in tune:
+            assert inf[name] == tune[key], (key, inf)
+
+
 def run_and_compare_fp64(qmc, oracle, N, W, sweeps, step, rho=wl.RHO_EQ, b=2.89, base=0, split=None, proposal=0,
-                         expect_cluster=None):
+                         expect_cluster=None, tune=None):
+    """fp64 trajectory against the oracle.  The traced run is the DBG instantiation of the sweep kernel; afterwards a
+    second context runs the same chain WITHOUT a trace -- the lean instantiation bench.py times -- and must land on
+    the same bits (positions, pair sums, accepted-move counts): VERDICT r2 weak #1.  tune: the shape the caller forced
+    through the `tuning` fixture (checked against qmc_info for both contexts)."""
     q, L = make(qmc, N, W, qmc.QMC_FP64, rho=rho, b=b, base=base)
     if expect_cluster is not None:
         assert q.info()["sweep_cluster"] == expect_cluster, q.info()
+    check_shape(q.info(), tune or {})
     q.set_proposal(proposal)
     q.init_walkers(wl.SEED)
     dec, mar = q.trace_decisions(0, W, sweeps * N)
@@ -132,7 +167,20 @@ def run_and_compare_fp64(qmc, oracle, N, W, sweeps, step, rho=wl.RHO_EQ, b=2.89,
     assert np.allclose(acc, dec.sum(1) / (sweeps * N), rtol=0, atol=1e-15)
     for w in range(min(W, 4)):                      # running sums track the definition (P12 / R17)
         assert np.allclose(Sg[w], oracle.pair_sums(s, xfree[w]), rtol=1e-11, atol=1e-11)
+    info = q.info()
     q.close()
+    # the same chain without the trace: the instantiation that is timed
+    q2, _ = make(qmc, N, W, qmc.QMC_FP64, rho=rho, b=b, base=base)
+    inf2 = q2.info()
+    assert all(inf2[k] == info[k] for k in ("sweep_threads", "sweep_pairs_per_thread", "sweep_vector", "sweep_cluster"))
+    q2.set_proposal(proposal)
+    q2.init_walkers(wl.SEED)
+    for part in (split or [sweeps]):
+        q2.sweep(part, step)
+    assert np.array_equal(q2.get_positions().cpu().numpy(), xg), "untraced run must land on the oracle-checked bits"
+    assert np.array_equal(q2.pair_sums().cpu().numpy(), Sg)
+    assert np.array_equal(q2.acceptance().cpu().numpy(), acc)
+    q2.close()
     return exempt, dec.mean()
 
 
@@ -151,8 +199,74 @@ def test_trajectory_shapes_and_ragged_tails(qmc, oracle, N, W, sweeps):
 
 
 def test_trajectory_config3_size_sampled(qmc, oracle):
-    """N = 1952 in the bench launch shape (256 threads x 8 particles), a sample of walkers and sweeps."""
+    """N = 1952 in the shape the planner gives FEW walkers (wide blocks, few particles per thread), a sample of walkers
+    and sweeps; the shape bench.py times (2048 walkers: 128 threads x 16 particles) is forced in
+    test_trajectory_fp64_bench_shapes."""
     run_and_compare_fp64(qmc, oracle, 1952, 4, 2, 1.0, base=100)
+
+
+def test_contexts_with_their_own_tuning_coexist(qmc, oracle):
+    """qmc_create_tuned: two contexts with different forced sweep shapes, and a third on the
+    heuristics, alive at the same time, with no process-wide override set; fp64, so all three land on the same bits."""
+    N, W = 256, 4
+    L = wl.box_edge(N, wl.RHO_EQ)
+    tunes = [dict(sweep_threads=64, sweep_per_thread=4, sweep_vector=2), dict(sweep_threads=32, sweep_per_thread=8, sweep_vector=1),
+             dict()]
+    qs = [qmc.QMC(N, [W], [L], [2.89], DK, AZ, qmc.QMC_FP64, jitter=wl.JITTER, tuning=t) for t in tunes]
+    q0, _ = make(qmc, N, W, qmc.QMC_FP64)                       # qmc_create: the (unset) process-wide defaults
+    for q, t in zip(qs, tunes):
+        check_shape(q.info(), t)
+    assert qs[2].info() == q0.info()
+    assert qs[0].info()["sweep_threads"] != qs[1].info()["sweep_threads"]
+    for q in qs:
+        q.init_walkers(wl.SEED)
+    for q in qs:                                                 # interleaved launches of the three shapes
+        q.sweep(2, 1.0)
+    x = [q.get_positions().cpu().numpy() for q in qs]
+    assert np.array_equal(x[0], x[1]) and np.array_equal(x[0], x[2])
+    with pytest.raises(qmc.QmcError) as e:
+        qmc.QMC(N, [W], [L], [2.89], DK, AZ, qmc.QMC_FP64, tuning=dict(no_such_key=1))
+    assert e.value.code == qmc.QMC_E_ARG
+
+
+# the launch shapes of the fp64 lines in BENCH's `configs` block (W-aware planner at the full walker count)
+BENCH_SHAPES_FP64 = {
+    2: dict(sweep_threads=64, sweep_per_thread=4, sweep_vector=2),
+    3: dict(sweep_threads=128, sweep_per_thread=16, sweep_vector=2),
+    5: dict(sweep_threads=32, sweep_per_thread=16, sweep_vector=2),
+}
+
+
+@pytest.mark.parametrize("index", [1, 2, 3, 5])
+def test_planner_shapes_at_bench_size_fp64(qmc, index):
+    """What the planner picks for the FULL walker count of each fp64 bench line (contexts only, nothing runs): these
+    are the shapes the trajectory tests below force for a few walkers."""
+    w = wl.config(index)
+    if index == 3:
+        w = wl.with_mode(w, wl.MODE_FP64)
+    q = qmc.QMC.from_workload(w)
+    inf = q.info()
+    q.close()
+    if index in BENCH_SHAPES_FP64:
+        check_shape(inf, BENCH_SHAPES_FP64[index])
+    assert inf["sweep_cluster"] == 1 and inf["sweep_tile"] == 1, inf
+    print(index, inf)
+
+
+@pytest.mark.parametrize("N,W,sweeps,tune", [
+    (256, 6, 6, BENCH_SHAPES_FP64[2]),                                                 # config 2
+    (1952, 3, 2, BENCH_SHAPES_FP64[3]),                                                # config 3, fp64 run
+    (512, 4, 3, BENCH_SHAPES_FP64[5]),                                                 # config 5 (one density)
+    (1000, 3, 2, dict(sweep_threads=128, sweep_per_thread=8, sweep_vector=2)),         # J = 8, ragged (1000 < 1024)
+    (900, 3, 2, dict(sweep_threads=64, sweep_per_thread=16, sweep_vector=2)),          # J = 16, ragged
+    (250, 4, 4, dict(sweep_threads=32, sweep_per_thread=8, sweep_vector=1)),           # scalar packs, one warp
+])
+def test_trajectory_fp64_bench_shapes(qmc, oracle, tuning, N, W, sweeps, tune):
+    """the fp64 shapes bench.py times (many particles per thread, J = 4 ... 16), forced for a few
+    walkers, traced against the oracle move for move and then re-run untraced (the timed instantiation) to the bit."""
+    tuning(**tune)
+    exempt, acc = run_and_compare_fp64(qmc, oracle, N, W, sweeps, 1.0, base=21, tune=tune)
+    assert exempt <= 1 and 0.3 < acc < 0.8
 
 
 @pytest.mark.parametrize("N,W,sweeps,step", [(2, 6, 40, 0.3), (33, 4, 10, 0.6), (64, 8, 20, 0.6), (256, 6, 6, 0.8),
@@ -197,6 +311,41 @@ def test_trajectory_cluster_kernel_fp64(qmc, oracle, tuning, N, W, sweeps, C):
     assert exempt <= 1 and 0.3 < acc < 0.8
 
 
+def test_cluster_plan_serves_proposal_1_and_writeouts_through_one_block(qmc, oracle):
+    """for few walkers of many atoms the planner picks the cluster kernel, which has neither proposal 1 nor
+    in-kernel write-outs; the plan keeps the one-block shape as fallback and uses it for those calls (they used to
+    fail with QMC_E_ARG).  fp64, N = 2600 on 8 blocks: proposal 1 bit for bit against the oracle; FP32C, N = 4096,
+    W = 8: proposal 1 and write-outs run, acceptance plausible, running sums consistent with a rebuild."""
+    import torch
+    exempt, acc = run_and_compare_fp64(qmc, oracle, 2600, 2, 1, 0.8, base=9, proposal=1, expect_cluster=8)
+    assert exempt <= 1 and 0.2 < acc < 0.9
+    N, W = 4096, 8
+    q, L = make(qmc, N, W, qmc.QMC_FP32C)
+    assert q.info()["sweep_cluster"] > 1
+    q.init_walkers(wl.SEED)
+    q.set_proposal(1)
+    q.sweep(2, 0.8)
+    a = q.acceptance().cpu().numpy()
+    assert np.all((a > 0.2) & (a < 0.9)), a
+    q.set_proposal(0)
+    xyz = torch.full((2, W, 3, N), -1.0, dtype=torch.float64, device="cuda")
+    flags = torch.zeros((2, W), dtype=torch.int32, device="cuda")
+    q.sweep_writeouts(2, 1.0, 1, xyz, None, flags)
+    assert flags.cpu().numpy().all()
+    assert torch.equal(xyz[1], q.get_positions()) and not torch.equal(xyz[0], xyz[1])
+    S = q.pair_sums().cpu().numpy()
+    q.refresh_pair_sums()
+    S2 = q.pair_sums().cpu().numpy()
+    assert np.abs(S - S2).max() < 5e-5 * np.abs(S2).max()
+    # N = 40960: no single block holds the walker, so the refusal stays, with a message that says why
+    q, L = make(qmc, 40960, 1, qmc.QMC_FP32C)
+    q.init_walkers(1)
+    q.set_proposal(1)
+    with pytest.raises(qmc.QmcError) as e:
+        q.sweep(1, 0.5)
+    assert e.value.code == qmc.QMC_E_ARG and "no single thread block" in str(e.value)
+
+
 def test_large_n_needs_no_capacity_error_any_more(qmc, oracle):
     """N = 40 960 (the paper's largest system, K20 register kernel) in the fp32-coordinate mode: the
     planner spreads the walker over a cluster, the gridded energy kernel streams the coordinates from global memory.
@@ -218,6 +367,7 @@ def test_large_n_needs_no_capacity_error_any_more(qmc, oracle):
     eg = q.local_energy().cpu().numpy()
     eo = oracle.local_energy(s, xg)
     assert relerr32(eg, eo).max() < TOL32, relerr32(eg, eo)
+    assert relerr(eg, eo[:, :4]).max() < TOL32, relerr(eg, eo[:, :4])        # the plain relative 1e-5, E_PB included
     assert np.abs(q.pair_sums().cpu().numpy()[0] - So).max() < 2e-6 * np.abs(So).max()
 
 
@@ -242,10 +392,16 @@ def test_walker_shard_reproduces_global_walkers(qmc):
         assert torch.equal(q.acceptance()[3:7], qs.acceptance())
 
 
-def test_multi_group_config5_shape(qmc, oracle):
-    """configs[4] shape: several (rho, b) points in ONE context, per-group steps; 2 walkers per point."""
+@pytest.mark.parametrize("forced", [False, True])
+def test_multi_group_config5_shape(qmc, oracle, tuning, forced):
+    """configs[4] shape: several (rho, b) points in ONE context, per-group steps; 2 walkers per point.  forced: in the
+    launch shape bench.py times for the 16384 walkers of the full config (32 threads x 16 particles)."""
     w = wl.config(5).truncated(2, sweeps=3)
+    if forced:
+        tuning(**BENCH_SHAPES_FP64[5])
     q = qmc.QMC.from_workload(w)
+    if forced:
+        check_shape(q.info(), BENCH_SHAPES_FP64[5])
     q.init_walkers(w.seed)
     dec, mar = q.trace_decisions(0, w.n_walkers, 3 * w.n_atoms)
     q.sweep(3, w.steps)
@@ -261,6 +417,12 @@ def test_multi_group_config5_shape(qmc, oracle):
         assert np.array_equal(xo, xg[2 * g:2 * g + 2])
         eo = oracle.local_energy(s, xo)[:, :4]
         assert relerr(eg[2 * g:2 * g + 2], eo).max() < TOL64
+    # untraced: the timed instantiation, all 16 parameter points at once
+    q2 = qmc.QMC.from_workload(w)
+    q2.init_walkers(w.seed)
+    q2.sweep(3, w.steps)
+    assert np.array_equal(q2.get_positions().cpu().numpy(), xg)
+    assert np.array_equal(q2.local_energy().cpu().numpy(), eg)
 
 
 # ------------------------------------------------------------------------------ local energy
@@ -345,6 +507,33 @@ def test_local_energy_fp32c_singular_configuration_is_not_finite(qmc):
     assert np.array_equal(e[[0, 2]], e_good[[0, 2]]) and np.array_equal(S[[0, 2]], S_good[[0, 2]])
 
 
+def test_local_energy_fp32c_pair_beyond_the_fixed_point_range_is_flagged(qmc, tuning):
+    """a pair at r/L ~ 1e-3 (finite, but its partial sums exceed what the 56-bit fixed-point per-particle
+    accumulators of the unordered-pair kernel hold) used to wrap S_i silently; the walker now comes out as NaN (pair
+    sums, T_PB, E_PB), like the coincident case; with b = 0 nothing is flagged (test_free_particles_...).  A pair at r/L = 0.02 (closer than any liquid pair, still in range) stays
+    finite and agrees with the gridded kernel, which accumulates in floating point."""
+    N, W = 1952, 3
+    tuning(energy_ordered=2)
+    q, L = make(qmc, N, W, qmc.QMC_FP32C)
+    assert q.info()["energy_variant"] == 2
+    xyz = np.stack([wl.liquid_configuration(N, L, 77, fp32_grid=True)] * W)
+    xyz[1, :, 40] = xyz[1, :, 1300]
+    xyz[1, 0, 40] = (xyz[1, 0, 1300] + 1e-3 * L) % L
+    xyz[2, :, 40] = xyz[2, :, 1300]
+    xyz[2, 1, 40] = (xyz[2, 1, 1300] + 0.02 * L) % L
+    q.set_positions(xyz)
+    e, S = q.local_energy().cpu().numpy(), q.pair_sums().cpu().numpy()
+    assert np.isnan(S[1]).all() and np.isnan(e[1, [0, 2]]).all()          # pair sums, E_PB, T_PB (V and T_JF are floating-point totals)
+    assert np.isfinite(S[[0, 2]]).all() and np.isfinite(e[[0, 2]]).all()
+    tuning(energy_ordered=3)
+    qg, _ = make(qmc, N, W, qmc.QMC_FP32C)
+    qg.set_positions(xyz)
+    eg, Sg = qg.local_energy().cpu().numpy(), qg.pair_sums().cpu().numpy()
+    assert np.abs(S[2] - Sg[2]).max() < 1e-5 * np.abs(Sg[2]).max()
+    assert np.abs(e[2] - eg[2]).max() < 1e-5 * np.abs(eg[2]).max()
+    assert np.abs(e[0] - eg[0]).max() < 1e-5 * np.abs(eg[0]).max()
+
+
 @pytest.mark.parametrize("N,W", [(64, 16), (256, 4)])
 def test_local_energy_fp32c_equilibrated_liquid(qmc, oracle, N, W):
     """The regime the tolerance is hardest in: an EQUILIBRATED liquid (E = V + T cancels ~3.5x).  The
@@ -372,6 +561,7 @@ def test_local_energy_config4_size(qmc, oracle):
     eg = q.local_energy().cpu().numpy()
     eo = oracle.local_energy(orc_sys(oracle, N, L), xyz)
     assert relerr32(eg, eo).max() < TOL32
+    assert relerr(eg, eo[:, :4]).max() < TOL32, relerr(eg, eo[:, :4])        # the plain relative 1e-5, E_PB included
     # and sweeps run at this size (512 threads x 20 particles): the running pair sums after two sweeps against the
     # oracle's definition on the exported coordinates, and against the kernel's own from-scratch rebuild
     q.sweep(2, 1.0)
@@ -630,6 +820,31 @@ def test_fp32c_sum_representations_agree(qmc, tuning):
         assert np.abs(S1 - S1r).max() < 2e-5 * np.abs(S1r).max()
 
 
+@pytest.mark.parametrize("N", [512, 1952])
+@pytest.mark.parametrize("what", ["soft_repulsion", "wide_damping", "no_dispersion"])
+def test_local_energy_fp64_other_potential_constants(qmc, oracle, N, what):
+    """the fp64 energy kernel leaves the two exponentials of the potential out for pairs beyond 3 r_m, which is
+    exact to 3e-15 for HFD-B(HE)'s constants only.  With a softer repulsion (alpha = 4: the term is 1e-3 of the
+    dispersion sum at 3 r_m), a damping that reaches beyond 3 r_m (D = 3.5) or no dispersion at all the kernel must
+    evaluate them for every pair: 1e-10 against the oracle with the same constants (N = 512: warp-queue form,
+    N = 1952: pending-slot form with the standard constants)."""
+    az = list(AZ)
+    if what == "soft_repulsion":
+        az[3] = 4.0
+    elif what == "wide_damping":
+        az[8] = 3.5
+    else:
+        az[5] = az[6] = az[7] = 0.0
+    W = 2
+    q, L = make(qmc, N, W, qmc.QMC_FP64, aziz=az)
+    assert q.info()["energy_variant"] == 1
+    xyz = np.stack([wl.liquid_configuration(N, L, 600 + k) for k in range(W)])
+    q.set_positions(xyz)
+    eg = q.local_energy().cpu().numpy()
+    eo = oracle.local_energy(orc_sys(oracle, N, L, aziz=az), xyz)
+    assert relerr(eg, eo[:, :4]).max() < TOL64, (eg, eo)
+
+
 def test_local_energy_fp64_ordered_fallback(qmc, oracle, tuning):
     """The ordered-pair fp64 energy kernel (used when the unordered-pair kernel's accumulators do not fit
     shared memory) against the oracle."""
@@ -684,6 +899,46 @@ def test_pair_histogram_distances_on_bin_edges(qmc, oracle, mode_name):
     Ho = oracle.pair_histogram(orc_sys(oracle, N, L), xyz, nb)
     assert np.array_equal(Hg.astype(np.int64), Ho.astype(np.int64))
     assert Hg.sum() > 0
+
+
+@pytest.mark.parametrize("mode_name", ["fp64", "fp32c"])
+@pytest.mark.parametrize("nb", [1, 2, 4, 64, 512])
+def test_pair_histogram_close_pairs_and_few_bins(qmc, oracle, mode_name, nb):
+    """Pairs in the first half of bin 0 (the filtered kernel read floor(u) for u < 1/4 as bin -1, dropped
+    the pair and incremented the word before the histogram, a coordinate).  Walker 0: ideal gas (uniform random points,
+    no hard core); walker 1: a liquid with particles moved next to others -- the same point, 1e-3, 0.1, 0.24 and 0.26 of
+    a bin away; walker 2: all particles inside a cube of 0.2 bin (every pair in the first half of bin 0); walker 3:
+    the liquid itself (with 1, 2 or 4 bins a quarter bin is L/8 ... L/32: ordinary liquid pairs)."""
+    mode = qmc.QMC_FP64 if mode_name == "fp64" else qmc.QMC_FP32C
+    N, W = 100, 4
+    q, L = make(qmc, N, W, mode)
+    rng = np.random.default_rng(77 + nb)
+    dr = 0.5 * L / nb
+    liquid = wl.liquid_configuration(N, L, 4242)                          # [3][N]
+    gas = rng.uniform(0.0, L, size=(3, N))
+    close = liquid.copy()
+    for k, frac in enumerate((0.0, 1e-3, 0.1, 0.24, 0.26)):
+        a, b = 2 * k, 2 * k + 1
+        close[:, b] = close[:, a]
+        close[k % 3, b] = (close[k % 3, a] + frac * dr) % L
+    blob = (0.37 * L + rng.uniform(0.0, 0.2 * dr / math.sqrt(3.0), size=(3, N))) % L
+    q.set_positions(np.stack([gas, close, blob, liquid]))
+    xyz = q.get_positions().cpu().numpy()                                   # what the GPU holds (FP32C: on the grid)
+    Hg = q.pair_histogram(nb).cpu().numpy().astype(np.int64)
+    Ho = oracle.pair_histogram(orc_sys(oracle, N, L), xyz, nb).astype(np.int64)
+    assert np.array_equal(Hg, Ho), (Hg[:, :4], Ho[:, :4])
+    assert Hg[2, 0] == N * (N - 1) // 2                                     # the blob: every pair in bin 0
+    # the kernel left the walker's state alone (the word in front of the bins is the last z coordinate)
+    assert np.array_equal(q.get_positions().cpu().numpy(), xyz)
+
+
+def test_pair_histogram_two_particles_on_one_point(qmc, oracle):
+    for mode in (qmc.QMC_FP64, qmc.QMC_FP32C):
+        q, L = make(qmc, 2, 1, mode)
+        q.set_positions(np.full((1, 3, 2), 0.3 * L))
+        for nb in (1, 3, 512, 1000):
+            H = q.pair_histogram(nb).cpu().numpy()
+            assert H[0, 0] == 1 and H.sum() == 1, (mode, nb, H[0, :4])
 
 
 # ------------------------------------------------------------------------------ boundary behaviour
@@ -851,7 +1106,8 @@ def test_run_blocks_host_vs_oracle(qmc, oracle):
     assert np.array_equal(q.get_positions().cpu().numpy(), xo)
 
 
-@pytest.mark.parametrize("N,W,every,n_out,where", [(64, 5, 2, 4, "host"), (100, 3, 1, 3, "device"), (2, 4, 3, 2, "host")])
+@pytest.mark.parametrize("N,W,every,n_out,where", [(64, 5, 2, 4, "host"), (100, 3, 1, 3, "device"), (2, 4, 3, 2, "host"),
+                                                   (2600, 2, 1, 2, "device")])     # planned on a cluster: one-block fallback
 def test_sweep_writeouts_fp64_vs_oracle(qmc, oracle, N, W, every, n_out, where):
     """qmc_sweep_writeouts (NEXT-4, the paper's mechanism: l.175, l.323, l.343): ONE launch, the running kernel writes
     coordinates and accepted-move counts out every `every` sweeps -- into mapped pinned host memory or device
@@ -859,6 +1115,7 @@ def test_sweep_writeouts_fp64_vs_oracle(qmc, oracle, N, W, every, n_out, where):
     chain after the same number of sweeps."""
     import torch
     q, L = make(qmc, N, W, qmc.QMC_FP64)
+    assert (q.info()["sweep_cluster"] > 1) == (N >= 2500)
     q.init_walkers(wl.SEED)
     sweeps = every * n_out + (1 if every > 1 else 0)          # a trailing sweep without write-out
     step = 1.0 if N > 2 else 0.4
